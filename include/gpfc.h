@@ -1,0 +1,177 @@
+/*
+ * gpfc.h -- C ABI of libgpfc.so: B200-native GPU phase folding + noise
+ * normalisation, the data-parallel hot path of GPFC (arXiv 2312.02063,
+ * "PAPER.md" below; line numbers refer to /root/reference/PAPER.md).
+ *
+ * What the path computes (one "fold" per (light curve, trial period) pair):
+ *   step 1  u = t - t0, x = u / P, phi = x - floor(x)      PAPER.md:87(1), :111 "First"
+ *   step 2  k = min(trunc(phi * nbins), nbins - 1)          PAPER.md:105, :111 "Secondly"
+ *   step 3  sum[k] += flux, count[k] += 1                   PAPER.md:111 "Thirdly"
+ *   step 5  mean[k] = sum[k] / count[k]                     PAPER.md:111 "Lastly"
+ *   normalise: out[k] = mu + (mean[k] - mu) / s, mu and s the mean and the
+ *           population standard deviation of mean[] over the non-empty bins;
+ *           empty bins get mu
+ * The phase formula is exactly the one above in IEEE fp64 with no FMA
+ * contraction (true division); the kernels use a reciprocal multiply with a
+ * guard band and fall back to the division wherever the two could differ, so
+ * bin indices are bit-identical to that formula.
+ *
+ * Conventions for every call
+ *   - Pointers marked "device" must be device-accessible memory of the
+ *     current CUDA device; pointers marked "host" are ordinary host memory.
+ *     All memory is owned by the caller.  Nothing is retained after the work
+ *     is enqueued, except the workspace registered with gpfc_set_workspace.
+ *   - Device-pointer calls are asynchronous on the calling thread's current
+ *     gpfc stream (gpfc_set_stream; default: the legacy default stream) and
+ *     never synchronise the host.  *_host calls are synchronous.
+ *   - Return value: a gpfc_status (0 = success).  On failure
+ *     gpfc_last_error() describes it; outputs are then unspecified.
+ *   - Sizes of 0 (n, nperiods, ncurves, nprofiles) are valid no-ops.
+ *   - nbins: 1 <= nbins <= GPFC_MAX_NBINS.  Any value is accepted; powers of
+ *     two take the fast path.
+ *   - Outputs are fully overwritten, layout row-major [curve][period][bin].
+ *   - Data conventions (cannot be checked on the host): a sample whose time
+ *     or flux is not finite is skipped (not counted); a period that is not
+ *     finite and positive yields an all-zero row (sum, count and norm).
+ *   - Sums are accumulated exactly in per-curve fixed point (DESIGN.md
+ *     "Accumulation"): for flux that is a multiple of 2^-s on the curve's
+ *     scale the sums are exact and independent of order.
+ *   - There is no CPU fallback: without a CUDA device every compute call
+ *     returns GPFC_ERR_CUDA.
+ */
+#ifndef GPFC_H
+#define GPFC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    GPFC_OK = 0,
+    GPFC_ERR_INVALID_ARG = 1,  /* NULL required pointer, negative size, bad range  */
+    GPFC_ERR_UNSUPPORTED = 2,  /* nbins out of range                               */
+    GPFC_ERR_WORKSPACE = 3,    /* registered workspace too small / allocation failed */
+    GPFC_ERR_CUDA = 4          /* CUDA runtime error (text in gpfc_last_error)     */
+} gpfc_status;
+
+#define GPFC_MAX_NBINS 4096
+
+/* gpfc_make_period_grid mode_flags: spacing | endpoint */
+enum { GPFC_GRID_UNIFORM_FREQUENCY = 0, GPFC_GRID_UNIFORM_PERIOD = 1 };
+enum { GPFC_GRID_ENDPOINT_INCLUSIVE = 0, GPFC_GRID_ENDPOINT_EXCLUSIVE = 2 };
+
+/* Library version string (static storage). */
+const char *gpfc_version(void);
+
+/* Text of the calling thread's last error (static thread-local storage; never NULL). */
+const char *gpfc_last_error(void);
+
+/* Set the calling thread's stream (a cudaStream_t passed as void*; NULL = legacy
+ * default stream).  Every later device-pointer call of this thread is enqueued on it. */
+int gpfc_set_stream(void *cuda_stream);
+
+/*
+ * Scratch memory.  The fold needs, per call, room for the pre-processed
+ * samples (u = t - t0 in fp64, fixed-point flux), per-curve and per-period
+ * tables: gpfc_workspace_bytes() returns an upper bound for a call of the given
+ * size.  If a workspace registered with gpfc_set_workspace() (device memory,
+ * 256-byte aligned, owned by the caller, must stay valid until the work that
+ * uses it has finished) is large enough it is used; otherwise the library
+ * allocates and frees scratch stream-ordered (cudaMallocAsync) inside the call.
+ * gpfc_set_workspace(NULL, 0) unregisters.  Per-thread, like the stream.
+ */
+size_t gpfc_workspace_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods, int nbins);
+int gpfc_set_workspace(void *dev_ptr, size_t bytes);
+
+/*
+ * Trial-period grid (Eq. 1 and "uniformly sample 100,000
+ * periods within [0.2, 1.0] days").  D = nperiods - 1 (inclusive) or nperiods
+ * (exclusive), at least 1.
+ *   frequency mode: f_j = 1/pmax + ((1/pmin - 1/pmax) * j) / D, periods_out[j] = 1 / f_j
+ *                   (ascending frequency, i.e. descending period)
+ *   period mode:    periods_out[j] = pmin + ((pmax - pmin) * j) / D
+ * every operation individually rounded to fp64 (no FMA).
+ * periods_out: device, fp64 [nperiods].  pmin <= 0, pmax < pmin, non-finite
+ * bounds or nperiods < 0 -> GPFC_ERR_INVALID_ARG.
+ */
+int gpfc_make_period_grid(double pmin, double pmax, int64_t nperiods, int mode_flags,
+                          double *periods_out);
+
+/* Eq. 1: N_sample = N_o * T / L.  Host-only helper for sizing the grid. */
+double gpfc_n_sample(double n_o, double t_window, double l_width);
+
+/*
+ * Fold one light curve over a set of trial periods (steps 1-3).
+ *   times    device fp64 [n]     sample times (any order, irregular allowed: PAPER.md:334)
+ *   flux     device fp32 [n]     detrended, median-subtracted relative flux
+ *   periods  device fp64 [nperiods]
+ *   t0       reference epoch subtracted from every time first
+ *   out_sum  device fp32 [nperiods][nbins]   per-bin flux sums   (may be NULL)
+ *   out_count device u32 [nperiods][nbins]   per-bin counts      (may be NULL)
+ */
+int gpfc_fold(const double *times, const float *flux, int64_t n,
+              const double *periods, int64_t nperiods, int nbins, double t0,
+              float *out_sum, uint32_t *out_count);
+
+/*
+ * Step 5 + noise normalisation of nprofiles folded profiles (PAPER.md:111
+ * "Lastly", :63).  sum, count: device [nprofiles][nbins]; out_norm: device fp32
+ * [nprofiles][nbins].  All-empty profile -> zeros; fewer than two non-empty
+ * bins or zero spread -> mu everywhere.  Arithmetic in fp64.
+ */
+int gpfc_normalize(const float *sum, const uint32_t *count, int64_t nprofiles, int nbins,
+                   float *out_norm);
+
+/*
+ * Batched fold, optionally fused with the normalisation.
+ *   times, flux  device, curves stored back to back: curve c is samples
+ *                offsets[c] .. offsets[c+1]-1
+ *   offsets      device int64 [ncurves + 1], non-decreasing, offsets[0] >= 0
+ *   n_total      number of elements in times / flux (>= offsets[ncurves]);
+ *                sizes the scratch, read on the host
+ *   periods      device fp64 [nperiods], shared by all curves
+ *   t0           device fp64 [ncurves], or NULL for 0.0
+ *   out_sum, out_count, out_norm   device [ncurves][nperiods][nbins]; any may
+ *                be NULL.  out_norm alone is the fused fold + normalise path:
+ *                sums and counts never leave shared memory.  out_norm is
+ *                computed from the exact sums, not from their fp32 roundings.
+ */
+int gpfc_fold_batch(const double *times, const float *flux, const int64_t *offsets,
+                    int64_t ncurves, int64_t n_total, const double *periods,
+                    int64_t nperiods, int nbins, const double *t0,
+                    float *out_sum, uint32_t *out_count, float *out_norm);
+
+/*
+ * Host-buffer convenience entry points (the end-to-end path): same
+ * arguments, but every pointer is HOST memory (pinned memory makes the copies
+ * faster but is not required).  The call allocates device buffers, copies the
+ * inputs in, runs the device path on the current stream, copies the requested
+ * outputs back and synchronises the stream before returning.
+ */
+int gpfc_make_period_grid_host(double pmin, double pmax, int64_t nperiods, int mode_flags,
+                               double *periods_out);
+int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *offsets,
+                         int64_t ncurves, int64_t n_total, const double *periods,
+                         int64_t nperiods, int nbins, const double *t0,
+                         float *out_sum, uint32_t *out_count, float *out_norm);
+
+/*
+ * Roofline calibration: runs the library's micro-kernels on
+ * the current stream and reports the measured peak rates of the units that
+ * bound the fold, so that bench.py can quote its denominator from the same run
+ * and clocks.  out (host, double[8]):
+ *   [0] conflict-free shared-memory atomic lane-updates / s (ATOMS.ADD + ATOMS.POPC.INC mix)
+ *   [1] fp64 (DMUL + DADD) pairs / s
+ *   [2] fold inner-loop point-periods / s with conflict-free bins (issue-bound ceiling)
+ *   [3..7] reserved (0)
+ * Synchronous.
+ */
+int gpfc_measure_peaks(double *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GPFC_H */

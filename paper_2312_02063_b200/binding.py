@@ -1,0 +1,216 @@
+"""Thin ctypes binding of libgpfc.so (include/gpfc.h) -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library; torch is used
+for device memory and streams.  Functions have the names of the C entry points.
+If the library is missing or fails to load this module raises: there is no CPU
+fallback and nothing here imports `oracle/`.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgpfc.so")
+
+GPFC_OK = 0
+GRID_UNIFORM_FREQUENCY = 0
+GRID_UNIFORM_PERIOD = 1
+GRID_ENDPOINT_INCLUSIVE = 0
+GRID_ENDPOINT_EXCLUSIVE = 2
+MAX_NBINS = 4096
+
+EXPORTS = [
+    "gpfc_version", "gpfc_last_error", "gpfc_set_stream", "gpfc_workspace_bytes",
+    "gpfc_set_workspace", "gpfc_make_period_grid", "gpfc_n_sample", "gpfc_fold",
+    "gpfc_normalize", "gpfc_fold_batch", "gpfc_make_period_grid_host",
+    "gpfc_fold_batch_host", "gpfc_measure_peaks",
+]
+
+
+class GpfcError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libgpfc.so (built in-tree by paper_2312_02063_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise GpfcError("libgpfc.so not found at %s: run `python -m paper_2312_02063_b200.build` "
+                        "(there is no CPU fallback)" % LIB_PATH)
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i64, i32, f64 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
+    L.gpfc_version.restype = ctypes.c_char_p
+    L.gpfc_last_error.restype = ctypes.c_char_p
+    L.gpfc_set_stream.argtypes = [vp]
+    L.gpfc_workspace_bytes.restype = ctypes.c_size_t
+    L.gpfc_workspace_bytes.argtypes = [i64, i64, i64, i32]
+    L.gpfc_set_workspace.argtypes = [vp, ctypes.c_size_t]
+    L.gpfc_make_period_grid.argtypes = [f64, f64, i64, i32, vp]
+    L.gpfc_make_period_grid_host.argtypes = [f64, f64, i64, i32, vp]
+    L.gpfc_n_sample.restype = f64
+    L.gpfc_n_sample.argtypes = [f64, f64, f64]
+    L.gpfc_fold.argtypes = [vp, vp, i64, vp, i64, i32, f64, vp, vp]
+    L.gpfc_normalize.argtypes = [vp, vp, i64, i32, vp]
+    fb = [vp, vp, vp, i64, i64, vp, i64, i32, vp, vp, vp, vp]
+    L.gpfc_fold_batch.argtypes = fb
+    L.gpfc_fold_batch_host.argtypes = fb
+    L.gpfc_measure_peaks.argtypes = [vp]
+    _lib = L
+    return L
+
+
+def _check(rc: int, what: str):
+    if rc != GPFC_OK:
+        raise GpfcError("%s failed (status %d): %s"
+                        % (what, rc, lib().gpfc_last_error().decode("utf-8", "replace")))
+
+
+def _dptr(t, dtype, name):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise GpfcError("%s must be a CUDA tensor" % name)
+    if t.dtype != dtype or not t.is_contiguous():
+        raise GpfcError("%s must be contiguous %s" % (name, dtype))
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _hptr(a, dtype, name):
+    if a is None:
+        return None
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or not a.is_contiguous():
+            raise GpfcError("%s must be a contiguous host tensor" % name)
+        return ctypes.c_void_p(a.data_ptr())
+    if not isinstance(a, np.ndarray) or a.dtype != dtype or not a.flags["C_CONTIGUOUS"]:
+        raise GpfcError("%s must be a contiguous numpy array of %s" % (name, dtype))
+    return ctypes.c_void_p(a.ctypes.data)
+
+
+def _use_current_stream():
+    lib().gpfc_set_stream(ctypes.c_void_p(torch.cuda.current_stream().cuda_stream))
+
+
+def gpfc_version() -> str:
+    return lib().gpfc_version().decode()
+
+
+def gpfc_n_sample(n_o: float, t_window: float, l_width: float) -> float:
+    return float(lib().gpfc_n_sample(n_o, t_window, l_width))
+
+
+def gpfc_workspace_bytes(ncurves: int, n_total: int, nperiods: int, nbins: int) -> int:
+    return int(lib().gpfc_workspace_bytes(ncurves, n_total, nperiods, nbins))
+
+
+def gpfc_set_workspace(ws) -> None:
+    """ws: a CUDA uint8 tensor kept alive by the caller, or None to unregister."""
+    if ws is None:
+        _check(lib().gpfc_set_workspace(None, 0), "gpfc_set_workspace")
+    else:
+        _check(lib().gpfc_set_workspace(ctypes.c_void_p(ws.data_ptr()), ws.numel() * ws.element_size()),
+               "gpfc_set_workspace")
+
+
+def gpfc_make_period_grid(pmin, pmax, nperiods, mode_flags=0, out=None, device="cuda"):
+    if out is None:
+        out = torch.empty(max(int(nperiods), 0), dtype=torch.float64, device=device)
+    _use_current_stream()
+    _check(lib().gpfc_make_period_grid(float(pmin), float(pmax), int(nperiods), int(mode_flags),
+                                       _dptr(out, torch.float64, "periods_out")),
+           "gpfc_make_period_grid")
+    return out
+
+
+def gpfc_fold(times, flux, periods, nbins, t0=0.0, out_sum=None, out_count=None):
+    n, npd = times.numel(), periods.numel()
+    dev = times.device
+    if out_sum is None:
+        out_sum = torch.empty((npd, nbins), dtype=torch.float32, device=dev)
+    if out_count is None:
+        out_count = torch.empty((npd, nbins), dtype=torch.int32, device=dev)
+    _use_current_stream()
+    _check(lib().gpfc_fold(_dptr(times, torch.float64, "times"), _dptr(flux, torch.float32, "flux"),
+                           n, _dptr(periods, torch.float64, "periods"), npd, int(nbins), float(t0),
+                           _dptr(out_sum, torch.float32, "out_sum"),
+                           _dptr(out_count, torch.int32, "out_count")), "gpfc_fold")
+    return out_sum, out_count
+
+
+def gpfc_normalize(sum_, count, out_norm=None):
+    nb = sum_.shape[-1]
+    nprof = sum_.numel() // nb if nb else 0
+    if out_norm is None:
+        out_norm = torch.empty_like(sum_)
+    _use_current_stream()
+    _check(lib().gpfc_normalize(_dptr(sum_, torch.float32, "sum"), _dptr(count, torch.int32, "count"),
+                                nprof, nb, _dptr(out_norm, torch.float32, "out_norm")),
+           "gpfc_normalize")
+    return out_norm
+
+
+def gpfc_fold_batch(times, flux, offsets, periods, nbins, t0=None, out_sum=None, out_count=None,
+                    out_norm=None, want=("sum", "count", "norm")):
+    """Device tensors in, device tensors out.  `want` selects which outputs are
+    allocated when none is passed in; want=("norm",) is the fused path."""
+    nc, npd, n_total = offsets.numel() - 1, periods.numel(), times.numel()
+    dev = times.device
+    shape = (nc, npd, nbins)
+    if out_sum is None and out_count is None and out_norm is None:
+        if "sum" in want:
+            out_sum = torch.empty(shape, dtype=torch.float32, device=dev)
+        if "count" in want:
+            out_count = torch.empty(shape, dtype=torch.int32, device=dev)
+        if "norm" in want:
+            out_norm = torch.empty(shape, dtype=torch.float32, device=dev)
+    _use_current_stream()
+    _check(lib().gpfc_fold_batch(
+        _dptr(times, torch.float64, "times"), _dptr(flux, torch.float32, "flux"),
+        _dptr(offsets, torch.int64, "offsets"), nc, n_total,
+        _dptr(periods, torch.float64, "periods"), npd, int(nbins),
+        _dptr(t0, torch.float64, "t0"), _dptr(out_sum, torch.float32, "out_sum"),
+        _dptr(out_count, torch.int32, "out_count"), _dptr(out_norm, torch.float32, "out_norm")),
+        "gpfc_fold_batch")
+    return out_sum, out_count, out_norm
+
+
+def gpfc_make_period_grid_host(pmin, pmax, nperiods, mode_flags=0):
+    out = np.empty(max(int(nperiods), 0), dtype=np.float64)
+    _use_current_stream()
+    _check(lib().gpfc_make_period_grid_host(float(pmin), float(pmax), int(nperiods),
+                                            int(mode_flags), _hptr(out, np.float64, "out")),
+           "gpfc_make_period_grid_host")
+    return out
+
+
+def gpfc_fold_batch_host(times, flux, offsets, periods, nbins, t0=None, out_sum=None,
+                         out_count=None, out_norm=None):
+    """Host buffers (numpy arrays or host torch tensors, pinned or not) in and
+    out; the outputs must be passed in (None = not wanted)."""
+    nc = offsets.shape[0] - 1
+    _use_current_stream()
+    _check(lib().gpfc_fold_batch_host(
+        _hptr(times, np.float64, "times"), _hptr(flux, np.float32, "flux"),
+        _hptr(offsets, np.int64, "offsets"), nc, times.shape[0],
+        _hptr(periods, np.float64, "periods"), periods.shape[0], int(nbins),
+        _hptr(t0, np.float64, "t0"), _hptr(out_sum, np.float32, "out_sum"),
+        _hptr(out_count, np.uint32, "out_count"), _hptr(out_norm, np.float32, "out_norm")),
+        "gpfc_fold_batch_host")
+    return out_sum, out_count, out_norm
+
+
+def gpfc_measure_peaks() -> dict:
+    out = (ctypes.c_double * 8)()
+    _use_current_stream()
+    _check(lib().gpfc_measure_peaks(out), "gpfc_measure_peaks")
+    return {"smem_atomic_lane_updates_per_s": out[0], "fp64_mul_add_pairs_per_s": out[1],
+            "fold_loop_pp_per_s": out[2]}

@@ -1,0 +1,306 @@
+// C ABI of libgpfc.so (include/gpfc.h): argument validation, scratch carving,
+// launches.  No compute happens on the host and there is no CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "common.cuh"
+
+namespace {
+
+struct ThreadState {
+    cudaStream_t stream = nullptr;
+    void *ws = nullptr;
+    size_t ws_bytes = 0;
+    char err[512] = "";
+};
+
+thread_local ThreadState g_ts;
+
+int fail(int code, const char *fmt, const char *detail = "")
+{
+    snprintf(g_ts.err, sizeof(g_ts.err), fmt, detail);
+    return code;
+}
+
+int cuda_fail(cudaError_t e, const char *where)
+{
+    snprintf(g_ts.err, sizeof(g_ts.err), "%s: %s", where, cudaGetErrorString(e));
+    return GPFC_ERR_CUDA;
+}
+
+size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+size_t scratch_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods)
+{
+    size_t b = 0;
+    b += align_up((size_t)n_total * sizeof(double));
+    b += align_up((size_t)n_total * sizeof(int));
+    b += align_up((size_t)ncurves * sizeof(gpfc::CurveMeta));
+    b += align_up((size_t)nperiods * sizeof(double));
+    b += align_up(2 * sizeof(int64_t));   // offsets of the single-curve call
+    return b + 256;
+}
+
+__global__ void set_offsets_kernel(int64_t *o, int64_t n)
+{
+    o[0] = 0;
+    o[1] = n;
+}
+
+// The device path shared by every fold entry point.
+int fold_device(const double *times, const float *flux, const int64_t *offsets, int64_t ncurves,
+                int64_t n_total, const double *periods, int64_t nperiods, int nbins,
+                const double *t0v, double t0_scalar, float *out_sum, uint32_t *out_count,
+                float *out_norm)
+{
+    if (ncurves < 0 || nperiods < 0 || n_total < 0)
+        return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
+    if (nbins < 1 || nbins > GPFC_MAX_NBINS)
+        return fail(GPFC_ERR_UNSUPPORTED, "nbins must be in [1, 4096]%s");
+    if (ncurves == 0 || nperiods == 0) return GPFC_OK;
+    if (!periods) return fail(GPFC_ERR_INVALID_ARG, "periods is NULL%s");
+    if (n_total > 0 && (!times || !flux)) return fail(GPFC_ERR_INVALID_ARG, "times/flux is NULL%s");
+    if (!out_sum && !out_count && !out_norm) return GPFC_OK;
+
+    cudaStream_t st = g_ts.stream;
+    size_t need = scratch_bytes(ncurves, n_total, nperiods);
+    char *base = nullptr;
+    bool own = false;
+    if (g_ts.ws && g_ts.ws_bytes >= need) {
+        base = static_cast<char *>(g_ts.ws);
+    } else {
+        void *p = nullptr;
+        cudaError_t e = cudaMallocAsync(&p, need, st);
+        if (e != cudaSuccess) {
+            cuda_fail(e, "scratch allocation");
+            return GPFC_ERR_WORKSPACE;
+        }
+        base = static_cast<char *>(p);
+        own = true;
+    }
+    char *cur = reinterpret_cast<char *>(align_up(reinterpret_cast<size_t>(base)));
+    gpfc::Scratch s;
+    s.u = reinterpret_cast<double *>(cur);
+    cur += align_up((size_t)n_total * sizeof(double));
+    s.q = reinterpret_cast<int *>(cur);
+    cur += align_up((size_t)n_total * sizeof(int));
+    s.meta = reinterpret_cast<gpfc::CurveMeta *>(cur);
+    cur += align_up((size_t)ncurves * sizeof(gpfc::CurveMeta));
+    s.rp = reinterpret_cast<double *>(cur);
+    cur += align_up((size_t)nperiods * sizeof(double));
+    int64_t *own_off = reinterpret_cast<int64_t *>(cur);
+
+    cudaError_t e = cudaSuccess;
+    if (!offsets) {   // single-curve entry point
+        set_offsets_kernel<<<1, 1, 0, st>>>(own_off, n_total);
+        offsets = own_off;
+    }
+    e = gpfc::launch_prep(times, flux, offsets, ncurves, t0v, t0_scalar, periods, nperiods, nbins,
+                          s, st);
+    if (e == cudaSuccess) {
+        gpfc::FoldArgs a;
+        a.u = s.u;
+        a.q = s.q;
+        a.meta = s.meta;
+        a.rp = s.rp;
+        a.periods = periods;
+        a.ncurves = ncurves;
+        a.nperiods = nperiods;
+        a.nbins = nbins;
+        a.out_sum = out_sum;
+        a.out_count = out_count;
+        a.out_norm = out_norm;
+        e = gpfc::launch_fold(a, st);
+    }
+    if (own) {
+        cudaError_t e2 = cudaFreeAsync(base, st);
+        if (e == cudaSuccess) e = e2;
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "fold launch");
+    return GPFC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *gpfc_version(void) { return "gpfc-b200 0.1 (sm_100a)"; }
+
+const char *gpfc_last_error(void) { return g_ts.err; }
+
+int gpfc_set_stream(void *cuda_stream)
+{
+    g_ts.stream = static_cast<cudaStream_t>(cuda_stream);
+    return GPFC_OK;
+}
+
+size_t gpfc_workspace_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods, int nbins)
+{
+    (void)nbins;
+    if (ncurves < 0 || n_total < 0 || nperiods < 0) return 0;
+    return scratch_bytes(ncurves, n_total, nperiods);
+}
+
+int gpfc_set_workspace(void *dev_ptr, size_t bytes)
+{
+    if (!dev_ptr && bytes) return fail(GPFC_ERR_INVALID_ARG, "workspace NULL with non-zero size%s");
+    g_ts.ws = dev_ptr;
+    g_ts.ws_bytes = dev_ptr ? bytes : 0;
+    return GPFC_OK;
+}
+
+double gpfc_n_sample(double n_o, double t_window, double l_width)
+{
+    return n_o * t_window / l_width;
+}
+
+static int grid_args_ok(double pmin, double pmax, int64_t nperiods)
+{
+    return nperiods >= 0 && pmin > 0.0 && pmax >= pmin && std::isfinite(pmax) &&
+           std::isfinite(pmin);
+}
+
+int gpfc_make_period_grid(double pmin, double pmax, int64_t nperiods, int mode_flags,
+                          double *periods_out)
+{
+    if (!grid_args_ok(pmin, pmax, nperiods))
+        return fail(GPFC_ERR_INVALID_ARG, "period grid: need 0 < pmin <= pmax, nperiods >= 0%s");
+    if (nperiods == 0) return GPFC_OK;
+    if (!periods_out) return fail(GPFC_ERR_INVALID_ARG, "periods_out is NULL%s");
+    cudaError_t e = gpfc::launch_grid(pmin, pmax, nperiods, mode_flags, periods_out, g_ts.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "grid launch");
+    return GPFC_OK;
+}
+
+int gpfc_fold(const double *times, const float *flux, int64_t n, const double *periods,
+              int64_t nperiods, int nbins, double t0, float *out_sum, uint32_t *out_count)
+{
+    if (n < 0) return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
+    return fold_device(times, flux, nullptr, 1, n, periods, nperiods, nbins, nullptr, t0, out_sum,
+                       out_count, nullptr);
+}
+
+int gpfc_normalize(const float *sum, const uint32_t *count, int64_t nprofiles, int nbins,
+                   float *out_norm)
+{
+    if (nprofiles < 0) return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
+    if (nbins < 1 || nbins > GPFC_MAX_NBINS)
+        return fail(GPFC_ERR_UNSUPPORTED, "nbins must be in [1, 4096]%s");
+    if (nprofiles == 0) return GPFC_OK;
+    if (!sum || !count || !out_norm) return fail(GPFC_ERR_INVALID_ARG, "NULL pointer%s");
+    cudaError_t e = gpfc::launch_normalize(sum, count, nprofiles, nbins, out_norm, g_ts.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "normalize launch");
+    return GPFC_OK;
+}
+
+int gpfc_fold_batch(const double *times, const float *flux, const int64_t *offsets,
+                    int64_t ncurves, int64_t n_total, const double *periods, int64_t nperiods,
+                    int nbins, const double *t0, float *out_sum, uint32_t *out_count,
+                    float *out_norm)
+{
+    if (ncurves > 0 && !offsets) return fail(GPFC_ERR_INVALID_ARG, "offsets is NULL%s");
+    return fold_device(times, flux, offsets, ncurves, n_total, periods, nperiods, nbins, t0, 0.0,
+                       out_sum, out_count, out_norm);
+}
+
+int gpfc_make_period_grid_host(double pmin, double pmax, int64_t nperiods, int mode_flags,
+                               double *periods_out)
+{
+    if (!grid_args_ok(pmin, pmax, nperiods))
+        return fail(GPFC_ERR_INVALID_ARG, "period grid: need 0 < pmin <= pmax, nperiods >= 0%s");
+    if (nperiods == 0) return GPFC_OK;
+    if (!periods_out) return fail(GPFC_ERR_INVALID_ARG, "periods_out is NULL%s");
+    cudaStream_t st = g_ts.stream;
+    double *d = nullptr;
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&d), (size_t)nperiods * 8, st);
+    if (e != cudaSuccess) return cuda_fail(e, "grid alloc");
+    e = gpfc::launch_grid(pmin, pmax, nperiods, mode_flags, d, st);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(periods_out, d, (size_t)nperiods * 8, cudaMemcpyDeviceToHost, st);
+    cudaFreeAsync(d, st);
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = e2;
+    if (e != cudaSuccess) return cuda_fail(e, "grid host path");
+    return GPFC_OK;
+}
+
+int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *offsets,
+                         int64_t ncurves, int64_t n_total, const double *periods,
+                         int64_t nperiods, int nbins, const double *t0, float *out_sum,
+                         uint32_t *out_count, float *out_norm)
+{
+    if (ncurves < 0 || nperiods < 0 || n_total < 0)
+        return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
+    if (nbins < 1 || nbins > GPFC_MAX_NBINS)
+        return fail(GPFC_ERR_UNSUPPORTED, "nbins must be in [1, 4096]%s");
+    if (ncurves == 0 || nperiods == 0) return GPFC_OK;
+    if (!offsets || !periods || (n_total > 0 && (!times || !flux)))
+        return fail(GPFC_ERR_INVALID_ARG, "NULL pointer%s");
+    cudaStream_t st = g_ts.stream;
+    const size_t nout = (size_t)ncurves * (size_t)nperiods * (size_t)nbins;
+    const size_t b_t = align_up((size_t)n_total * 8), b_f = align_up((size_t)n_total * 4);
+    const size_t b_o = align_up((size_t)(ncurves + 1) * 8), b_p = align_up((size_t)nperiods * 8);
+    const size_t b_t0 = t0 ? align_up((size_t)ncurves * 8) : 0;
+    const size_t b_out = align_up(nout * 4);
+    size_t total = b_t + b_f + b_o + b_p + b_t0 + 256;
+    total += (out_sum ? b_out : 0) + (out_count ? b_out : 0) + (out_norm ? b_out : 0);
+    char *base = nullptr;
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&base), total, st);
+    if (e != cudaSuccess) {
+        cuda_fail(e, "device buffer allocation");
+        return GPFC_ERR_WORKSPACE;
+    }
+    char *cur = base;
+    double *d_t = reinterpret_cast<double *>(cur); cur += b_t;
+    float *d_f = reinterpret_cast<float *>(cur); cur += b_f;
+    int64_t *d_o = reinterpret_cast<int64_t *>(cur); cur += b_o;
+    double *d_p = reinterpret_cast<double *>(cur); cur += b_p;
+    double *d_t0 = nullptr;
+    if (t0) { d_t0 = reinterpret_cast<double *>(cur); cur += b_t0; }
+    float *d_sum = nullptr, *d_norm = nullptr;
+    uint32_t *d_cnt = nullptr;
+    if (out_sum) { d_sum = reinterpret_cast<float *>(cur); cur += b_out; }
+    if (out_count) { d_cnt = reinterpret_cast<uint32_t *>(cur); cur += b_out; }
+    if (out_norm) { d_norm = reinterpret_cast<float *>(cur); cur += b_out; }
+
+    int rc = GPFC_OK;
+    if (n_total > 0) {
+        e = cudaMemcpyAsync(d_t, times, (size_t)n_total * 8, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(d_f, flux, (size_t)n_total * 4, cudaMemcpyHostToDevice, st);
+    }
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(d_o, offsets, (size_t)(ncurves + 1) * 8, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(d_p, periods, (size_t)nperiods * 8, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && t0)
+        e = cudaMemcpyAsync(d_t0, t0, (size_t)ncurves * 8, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        rc = fold_device(d_t, d_f, d_o, ncurves, n_total, d_p, nperiods, nbins, d_t0, 0.0, d_sum,
+                         d_cnt, d_norm);
+        if (rc == GPFC_OK) {
+            if (out_sum) e = cudaMemcpyAsync(out_sum, d_sum, nout * 4, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess && out_count)
+                e = cudaMemcpyAsync(out_count, d_cnt, nout * 4, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess && out_norm)
+                e = cudaMemcpyAsync(out_norm, d_norm, nout * 4, cudaMemcpyDeviceToHost, st);
+        }
+    }
+    cudaFreeAsync(base, st);
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    if (rc != GPFC_OK) return rc;
+    if (e == cudaSuccess) e = e2;
+    if (e != cudaSuccess) return cuda_fail(e, "host-buffer fold");
+    return GPFC_OK;
+}
+
+int gpfc_measure_peaks(double *out)
+{
+    if (!out) return fail(GPFC_ERR_INVALID_ARG, "out is NULL%s");
+    cudaError_t e = gpfc::measure_peaks(out, g_ts.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "measure_peaks");
+    return GPFC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,152 @@
+// Shared declarations of the CUDA path of libgpfc (sm_100a).  Not used by, and
+// not using, anything under oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+
+#include "../../include/gpfc.h"
+
+namespace gpfc {
+
+// Per-curve table written by the prepass (prep.cu) and read by the fold.
+struct CurveMeta {
+    long long start;   // first compacted sample of this curve in the u / q scratch arrays
+    int n_valid;       // samples with finite time and flux (compacted to the front)
+    int shift;         // fixed-point exponent s: q = rint((flux - center) * 2^s)
+    double center;     // per-curve constant removed before quantisation (0 for centred input)
+    double inv_scale;  // 2^-s
+    double umin;       // min / max of u = t - t0 over the valid samples
+    double umax;
+};
+
+// Scratch carved out of the workspace for one gpfc_fold_batch call.
+struct Scratch {
+    double *u;         // [n_total]  t - t0, valid samples compacted per curve
+    int *q;            // [n_total]  fixed-point flux
+    CurveMeta *meta;   // [ncurves]
+    double *rp;        // [nperiods] RN(1/P) * nbins, NaN for a period that is not finite-positive
+};
+
+struct FoldArgs {
+    const double *u;
+    const int *q;
+    const CurveMeta *meta;
+    const double *rp;
+    const double *periods;
+    long long ncurves;
+    long long nperiods;
+    int nbins;
+    float *out_sum;
+    uint32_t *out_count;
+    float *out_norm;
+};
+
+// ---- exact bin of one sample: the formula of include/gpfc.h, every operation
+// rounded once (intrinsics, so nothing can be contracted into an FMA).
+// PAPER.md:111 "First", "Secondly".
+__device__ __forceinline__ int exact_bin(double u, double period, int nbins)
+{
+    double x = __ddiv_rn(u, period);
+    double phi = __dsub_rn(x, floor(x));
+    double scaled = __dmul_rn(phi, (double)nbins);
+    long long k = (long long)scaled;   // truncation; scaled >= 0
+    if (k >= nbins) k = nbins - 1;
+    return (int)k;
+}
+
+__device__ __forceinline__ bool period_ok(double p)
+{
+    return (p > 0.0) && (p < CUDART_INF);   // false for NaN, <= 0, +inf
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ int warp_sum_int(int v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// One folded profile held in shared memory as nbins 8-byte slots
+// {int32 fixed-point sum, uint32 count}.  A whole warp converts it, writes the
+// requested outputs and leaves the slots zeroed.
+//   out_sum[k]   = (float)(Q * 2^-s + count * center)
+//   out_norm[k]  = mu + (m[k] - mu) / s, fp64, population std over
+//                  the non-empty bins; empty bins -> mu; K = 0 -> 0; K < 2 or s = 0 -> mu
+__device__ __forceinline__ void emit_profile(unsigned long long *slots, int nbins, int lane,
+                                             double inv_scale, double center, bool zero_row,
+                                             float *out_sum, uint32_t *out_count,
+                                             float *out_norm)
+{
+    double acc = 0.0;
+    int kk = 0;
+    double *mslots = reinterpret_cast<double *>(slots);
+    for (int k = lane; k < nbins; k += 32) {
+        unsigned long long s = slots[k];
+        int qsum = (int)(unsigned)(s & 0xffffffffull);
+        unsigned cnt = (unsigned)(s >> 32);
+        if (zero_row) {
+            qsum = 0;
+            cnt = 0;
+        }
+        double sf = __dadd_rn(__dmul_rn((double)qsum, inv_scale),
+                              __dmul_rn((double)cnt, center));
+        if (out_sum) out_sum[k] = (float)sf;
+        if (out_count) out_count[k] = cnt;
+        if (out_norm) {
+            double m = CUDART_NAN;
+            if (cnt > 0) {
+                m = __ddiv_rn(sf, (double)cnt);
+                acc += m;
+                kk += 1;
+            }
+            mslots[k] = m;
+        } else {
+            slots[k] = 0ull;
+        }
+    }
+    if (!out_norm) return;
+    __syncwarp();
+    acc = warp_sum(acc);
+    kk = warp_sum_int(kk);
+    double mu = (kk > 0) ? __ddiv_rn(acc, (double)kk) : 0.0;
+    double vacc = 0.0;
+    for (int k = lane; k < nbins; k += 32) {
+        double m = mslots[k];
+        if (m == m) {
+            double d = __dsub_rn(m, mu);
+            vacc += __dmul_rn(d, d);
+        }
+    }
+    vacc = warp_sum(vacc);
+    double sd = (kk > 0) ? sqrt(__ddiv_rn(vacc, (double)kk)) : 0.0;
+    bool flat = (kk < 2) || !(sd > 0.0);
+    for (int k = lane; k < nbins; k += 32) {
+        double m = mslots[k];
+        double o = mu;
+        if (!flat && m == m) o = __dadd_rn(mu, __ddiv_rn(__dsub_rn(m, mu), sd));
+        out_norm[k] = (float)o;
+        slots[k] = 0ull;
+    }
+}
+
+// launchers (defined in the .cu files)
+cudaError_t launch_prep(const double *times, const float *flux, const int64_t *offsets,
+                        long long ncurves, const double *t0, double t0_scalar,
+                        const double *periods, long long nperiods, int nbins, Scratch s,
+                        cudaStream_t st);
+cudaError_t launch_fold(const FoldArgs &a, cudaStream_t st);
+cudaError_t launch_normalize(const float *sum, const uint32_t *count, long long nprofiles,
+                             int nbins, float *out, cudaStream_t st);
+cudaError_t launch_grid(double pmin, double pmax, long long nperiods, int mode_flags,
+                        double *out, cudaStream_t st);
+cudaError_t measure_peaks(double *out_host, cudaStream_t st);
+
+}  // namespace gpfc

@@ -1,0 +1,154 @@
+// Roofline calibration micro-kernels (gpfc_measure_peaks): the
+// measured peak rates of the units that bound the fold on this GPU, in this run,
+// at these clocks.
+//   [0] conflict-free shared-memory atomic lane-updates/s: every lane owns a bank,
+//       half ATOMS.ADD, half ATOMS.POPC.INC, addresses precomputed, no other work
+//   [1] fp64 DMUL + DADD(round-down) pairs/s
+//   [2] the fold's inner loop (DMUL, DADD.RM, bin/address, guard, 2 atomics) with
+//       lane-private columns and samples in registers: the issue-bound ceiling of
+//       the main loop, with no loads, epilogue or barriers
+#include "common.cuh"
+
+namespace gpfc {
+
+namespace {
+
+extern __shared__ __align__(16) unsigned char peaks_smem[];
+
+__global__ void __launch_bounds__(1024, 1) peak_atoms_kernel(int iters, unsigned *sink)
+{
+    unsigned *h = reinterpret_cast<unsigned *>(peaks_smem);   // [rows][32]
+    constexpr int ROWS = 1024;
+    const int lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < ROWS * 32; i += blockDim.x) h[i] = 0;
+    __syncthreads();
+    unsigned idx[8];
+    unsigned s = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 12345u;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        s = s * 1664525u + 1013904223u;
+        idx[k] = ((s >> 8) % ROWS) * 32 + lane;
+    }
+    const unsigned v = lane + 1;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; k += 2) {
+            atomicAdd(&h[idx[k]], v);
+            atomicAdd(&h[idx[k + 1]], 1u);
+        }
+    }
+    __syncthreads();
+    unsigned acc = 0;
+    for (int i = threadIdx.x; i < ROWS * 32; i += blockDim.x) acc += h[i];
+    if (acc == 0xdeadbeefu) sink[0] = acc;
+}
+
+__global__ void __launch_bounds__(1024, 1) peak_fp64_kernel(int iters, double seed, double *sink)
+{
+    double u[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) u[k] = seed * (double)(threadIdx.x + 32 * k + 1);
+    double r = 1.0 + seed;
+    const double M = 6755399441055744.0 / 16777216.0;
+    unsigned acc = 0;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            double y = __dmul_rn(u[k], r);
+            double m = __dadd_rd(y, M);
+            acc ^= (unsigned)__double2loint(m);
+        }
+        r = __longlong_as_double(__double_as_longlong(r) + 1);
+    }
+    if (acc == 0xdeadbeefu) sink[0] = (double)acc;
+}
+
+__global__ void __launch_bounds__(1024, 1) peak_loop_kernel(int nper, double seed, unsigned *sink)
+{
+    constexpr int NBLOG = 8, NB = 256, KS = 4;
+    int *H = reinterpret_cast<int *>(peaks_smem);   // [2][NB][32]
+    const int lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < 2 * NB * 32; i += blockDim.x) H[i] = 0;
+    __syncthreads();
+    double u[KS];
+    int q[KS];
+#pragma unroll
+    for (int k = 0; k < KS; ++k) {
+        u[k] = 0.020433 * (double)(blockIdx.x * 4096 + k * 1024 + threadIdx.x) + seed;
+        q[k] = (int)threadIdx.x - 500 + k;
+    }
+    const double MAGIC = 6755399441055744.0 / (double)(1ull << (32 - NBLOG));
+    unsigned gmin = 0xffffffffu;
+    double r = 256.0;
+    for (int p = 0; p < nper; ++p) {
+#pragma unroll
+        for (int k = 0; k < KS; ++k) {
+            double y = __dmul_rn(u[k], r);
+            double mm = __dadd_rd(y, MAGIC);
+            unsigned lo = (unsigned)__double2loint(mm);
+            unsigned bin = lo >> (32 - NBLOG);
+            gmin = min(gmin, lo * (unsigned)NB + (unsigned)NB);
+            int *hs = H + bin * 32 + lane;
+            atomicAdd(hs, q[k]);
+            atomicAdd(reinterpret_cast<unsigned *>(hs + NB * 32), 1u);
+        }
+        r += 0.00048828125;
+    }
+    __syncthreads();
+    unsigned acc = gmin;
+    for (int i = threadIdx.x; i < 2 * NB * 32; i += blockDim.x) acc += (unsigned)H[i];
+    if (acc == 0xdeadbeefu) sink[0] = acc;
+}
+
+}  // namespace
+
+cudaError_t measure_peaks(double *out, cudaStream_t st)
+{
+    for (int i = 0; i < 8; ++i) out[i] = 0.0;
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    void *sink = nullptr;
+    cudaError_t e = cudaMalloc(&sink, 256);
+    if (e != cudaSuccess) return e;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a);
+    cudaEventCreate(&b);
+    const size_t smem_atoms = 1024 * 32 * 4, smem_loop = 2 * 256 * 32 * 4;
+    cudaFuncSetAttribute(peak_atoms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)smem_atoms);
+    cudaFuncSetAttribute(peak_loop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)smem_loop);
+    const int iters = 4000, nper = 4000;
+    for (int which = 0; which < 3; ++which) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; ++rep) {
+            cudaEventRecord(a, st);
+            if (which == 0)
+                peak_atoms_kernel<<<sms, 1024, smem_atoms, st>>>(iters, (unsigned *)sink);
+            else if (which == 1)
+                peak_fp64_kernel<<<sms * 2, 1024, 0, st>>>(iters, 1e-3, (double *)sink);
+            else
+                peak_loop_kernel<<<sms, 1024, smem_loop, st>>>(nper, 0.25, (unsigned *)sink);
+            cudaEventRecord(b, st);
+            e = cudaEventSynchronize(b);
+            if (e != cudaSuccess) break;
+            float ms = 0;
+            cudaEventElapsedTime(&ms, a, b);
+            if (rep > 0 && ms < best) best = ms;
+        }
+        if (e != cudaSuccess) break;
+        double units = 0;
+        if (which == 0) units = (double)sms * 1024 * iters * 8.0;
+        if (which == 1) units = (double)sms * 2 * 1024 * iters * 8.0;
+        if (which == 2) units = (double)sms * 1024 * nper * 4.0;
+        out[which] = units / (best * 1e-3);
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    cudaFree(sink);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    return e;
+}
+
+}  // namespace gpfc

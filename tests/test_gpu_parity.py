@@ -1,0 +1,243 @@
+"""GPU parity tests (-m gpu): the CUDA path through the C ABI against the CPU
+oracle, element by element, on the same seeded inputs.
+
+Bars (BASELINE.json north_star): bin counts bit-exact; bin means within 1e-6
+absolute; normalised profiles within 1e-4 * max(1, |ref|) (reading R14).  For the
+config inputs (flux on the 2^-24 lattice) the fixed-point sums are exact, so the
+fp32 sums are compared bit for bit as well.
+"""
+import numpy as np
+import pytest
+
+from paper_2312_02063_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def gp():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2312_02063_b200 import binding
+    binding.lib()          # must load: no fallback
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_gpu(gp, w, periods, t0=None, want=("sum", "count", "norm")):
+    s, c, nrm = gp.gpfc_fold_batch(dev(w.times), dev(w.flux), dev(w.offsets), dev(periods),
+                                   w.nbins, t0=None if t0 is None else dev(t0), want=want)
+    torch.cuda.synchronize()
+    out = {}
+    out["sum"] = None if s is None else s.cpu().numpy()
+    out["count"] = None if c is None else c.cpu().numpy().view(np.uint32)
+    out["norm"] = None if nrm is None else nrm.cpu().numpy()
+    return out
+
+
+def check(g, r, exact_sums=False):
+    assert np.array_equal(g["count"], r["count"]), "bin counts differ"
+    cnt = np.maximum(r["count"], 1).astype(np.float64)
+    mean_g = g["sum"].astype(np.float64) / cnt
+    mean_r = r["sum64"] / cnt
+    assert np.max(np.abs(mean_g - mean_r), initial=0.0) <= 1e-6
+    if exact_sums:
+        assert np.array_equal(g["sum"], r["sum"]), "fp32 sums differ on lattice input"
+    if g.get("norm") is not None:
+        ref = r["norm64"]
+        err = np.abs(g["norm"].astype(np.float64) - ref)
+        tol = 1e-4 * np.maximum(1.0, np.abs(ref))
+        assert np.all(err <= tol), "normalised profile off by %g" % float((err / tol).max())
+
+
+def test_grid_bit_identical(gp, ref):
+    for mode in (0, 1, 2, 3):
+        for (pmin, pmax, n) in [(0.2, 1.0, 2000), (0.2, 1.0, 1), (0.25, 0.5, 2), (0.2, 1.0, 100000),
+                                (0.3, 17.0, 12345)]:
+            g = gp.gpfc_make_period_grid(pmin, pmax, n, mode).cpu().numpy()
+            r = ref.make_period_grid(pmin, pmax, n, mode)
+            assert np.array_equal(g, r), (mode, pmin, pmax, n)
+    h = gp.gpfc_make_period_grid_host(0.2, 1.0, 5000, 0)
+    assert np.array_equal(h, ref.make_period_grid(0.2, 1.0, 5000, 0))
+    assert gp.gpfc_make_period_grid(0.2, 1.0, 0).numel() == 0
+    with pytest.raises(gp.GpfcError):
+        gp.gpfc_make_period_grid(-1.0, 1.0, 10)
+    assert int(gp.gpfc_n_sample(2, 4 * 365, 0.03)) == 97333
+
+
+def test_hand_vectors_on_gpu(gp):
+    """The same hand-worked dyadic vectors the oracle is pinned with."""
+    import json, os
+    g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "hand_vectors.json")))
+    t = dev(np.array(g["times"], np.float64))
+    f = dev(np.array(g["flux"], np.float32))
+    for case in g["cases"]:
+        s, c = gp.gpfc_fold(t, f, dev(np.array([case["period"]])), g["nbins"], t0=case["t0"])
+        assert c.cpu().tolist()[0] == case["count"], case
+        assert s.cpu().tolist()[0] == case["sum"], case
+    nz = g["normalize"]
+    out = gp.gpfc_normalize(dev(np.array([nz["sum"]], np.float32)),
+                            dev(np.array([nz["count"]], np.int32)))
+    assert np.allclose(out.cpu().numpy()[0], nz["out"], rtol=0, atol=1e-6)
+
+
+def test_config0_full(gp, ref):
+    w = workloads.config0()
+    periods = ref.make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode)
+    g = run_gpu(gp, w, periods)
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, w.nbins)
+    check(g, r, exact_sums=True)
+
+
+@pytest.mark.parametrize("nbins", [32, 64, 128, 256, 512, 1024, 2048, 4096])
+def test_pow2_nbins_kepler_slice(gp, ref, nbins):
+    """Config-1 curve (65,000 samples: many tiles + ragged tail) over a slice of the
+    grid that includes cadence-commensurate (degenerate) periods; 37 periods is not
+    a multiple of any period-group size, so the ragged last group is exercised."""
+    w = workloads.config1(nperiods=37)
+    grid = ref.make_period_grid(w.pmin, w.pmax, 200000, w.grid_mode)
+    idx = np.linspace(0, 199999, 30).astype(int)
+    dt = workloads.KEPLER_CADENCE_D
+    periods = np.concatenate([grid[idx], [10 * dt, 12 * dt, 16 * dt, 20 * dt, 0.5, 0.25, 1.0]])
+    w.nbins = nbins
+    g = run_gpu(gp, w, periods)
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
+    check(g, r, exact_sums=True)
+
+
+@pytest.mark.parametrize("nbins", [1, 2, 7, 16, 100, 1000, 4095])
+def test_generic_nbins(gp, ref, nbins):
+    w = workloads.config0(nperiods=25)
+    w.nbins = nbins
+    periods = ref.make_period_grid(w.pmin, w.pmax, 25, w.grid_mode)
+    g = run_gpu(gp, w, periods)
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
+    check(g, r, exact_sums=True)
+
+
+@pytest.mark.parametrize("nbins", [64, 100, 256])
+def test_ragged_batch_edge_cases(gp, ref, nbins):
+    """Empty and tiny curves, irregular times, negative t - t0, non-finite samples,
+    invalid periods, per-curve t0, flux off the lattice."""
+    w = workloads.ragged_batch(nbins=nbins)
+    periods = ref.make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode)
+    periods[3] = np.nan
+    periods[4] = 0.0
+    periods[5] = -0.5
+    periods[6] = np.inf
+    periods[7] = 1e-9            # x far outside the fast range
+    periods[8] = 1e9
+    t0 = np.linspace(-1.0, 2.0, w.ncurves)
+    g = run_gpu(gp, w, periods, t0=t0)
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins, t0=t0)
+    check(g, r)
+    for j in (3, 4, 5, 6):
+        assert not g["count"][:, j].any() and not g["sum"][:, j].any() and not g["norm"][:, j].any()
+    # t0 = NULL
+    g0 = run_gpu(gp, w, periods)
+    r0 = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
+    check(g0, r0)
+
+
+def test_guard_band_samples_match_division(gp, ref):
+    """Samples that sit exactly on bin edges (t = k P / nb, t = t0) and their
+    fp64 neighbours: the reciprocal fast path must fall back to the division."""
+    nb = 256
+    rng = np.random.default_rng(5)
+    periods = np.concatenate([rng.uniform(0.2, 1.0, 30), [0.5, 0.25, 0.75, 1.0, 0.3]])
+    ts = [np.zeros(3)]
+    for p in periods[:12]:
+        k = rng.integers(0, 200000, 400)
+        e = (k * p) / nb
+        ts += [e, np.nextafter(e, np.inf), np.nextafter(e, -np.inf), k.astype(np.float64) * p]
+    t = np.sort(np.concatenate(ts))
+    f = rng.integers(-1000, 1000, t.shape[0]).astype(np.float32) * np.float32(2.0 ** -20)
+    w = workloads._pack("edges", -1, [(t, f, None)], 0.2, 1.0, periods.shape[0], nb, False)
+    for nbins in (64, 256, 4096):
+        w.nbins = nbins
+        g = run_gpu(gp, w, periods)
+        r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
+        check(g, r, exact_sums=True)
+
+
+def test_uncentred_flux_is_centred_internally(gp, ref):
+    """Flux around 1.0 (not median-subtracted): the library removes a per-curve
+    constant before quantising; means still agree to 1e-6."""
+    w = workloads.config0(nperiods=40)
+    w.flux = (w.flux + np.float32(1.0)).astype(np.float32)
+    periods = ref.make_period_grid(w.pmin, w.pmax, 40, w.grid_mode)
+    g = run_gpu(gp, w, periods, want=("sum", "count"))
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, w.nbins)
+    check(g, r)
+
+
+def test_batch_configs_scaled(gp, ref):
+    """Config 2 and 4 shapes with fewer curves / periods (full parity)."""
+    w2 = workloads.config2(ncurves=3, nperiods=40)
+    p2 = ref.make_period_grid(w2.pmin, w2.pmax, 40, w2.grid_mode)
+    check(run_gpu(gp, w2, p2), ref.fold_batch(w2.times, w2.flux, w2.offsets, p2, w2.nbins),
+          exact_sums=True)
+    w4 = workloads.config4(ncurves=5, nperiods=50)
+    p4 = ref.make_period_grid(w4.pmin, w4.pmax, 50, w4.grid_mode)
+    g4 = run_gpu(gp, w4, p4, want=("norm",))         # fused: only the normalised profile
+    r4 = ref.fold_batch(w4.times, w4.flux, w4.offsets, p4, w4.nbins)
+    err = np.abs(g4["norm"].astype(np.float64) - r4["norm64"])
+    assert np.all(err <= 1e-4 * np.maximum(1.0, np.abs(r4["norm64"])))
+    assert g4["sum"] is None and g4["count"] is None
+
+
+def test_single_curve_fold_and_normalize_entry_points(gp, ref):
+    w = workloads.config0(nperiods=64)
+    periods = ref.make_period_grid(w.pmin, w.pmax, 64, w.grid_mode)
+    s, c = gp.gpfc_fold(dev(w.times), dev(w.flux), dev(periods), w.nbins, t0=0.37)
+    nrm = gp.gpfc_normalize(s, c)
+    torch.cuda.synchronize()
+    rs, rc, rs64 = ref.fold(w.times, w.flux, periods, w.nbins, t0=0.37)
+    assert np.array_equal(c.cpu().numpy().view(np.uint32), rc)
+    assert np.array_equal(s.cpu().numpy(), rs)
+    rn = ref.normalize(rs, rc, want64=True)[1]
+    err = np.abs(nrm.cpu().numpy().astype(np.float64) - rn)
+    assert np.all(err <= 1e-4 * np.maximum(1.0, np.abs(rn)))
+
+
+def test_host_entry_point_and_workspace(gp, ref):
+    w = workloads.config2(ncurves=2, nperiods=24)
+    periods = ref.make_period_grid(w.pmin, w.pmax, 24, w.grid_mode)
+    shape = (w.ncurves, 24, w.nbins)
+    s = np.empty(shape, np.float32)
+    c = np.empty(shape, np.uint32)
+    nrm = np.empty(shape, np.float32)
+    gp.gpfc_fold_batch_host(w.times, w.flux, w.offsets, periods, w.nbins, out_sum=s, out_count=c,
+                            out_norm=nrm)
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, w.nbins)
+    check({"sum": s, "count": c, "norm": nrm}, r, exact_sums=True)
+    # caller-owned workspace
+    need = gp.gpfc_workspace_bytes(w.ncurves, w.n_total, 24, w.nbins)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    gp.gpfc_set_workspace(ws)
+    try:
+        g = run_gpu(gp, w, periods)
+    finally:
+        gp.gpfc_set_workspace(None)
+    check(g, r, exact_sums=True)
+
+
+def test_empty_and_error_paths(gp):
+    e64 = torch.empty(0, dtype=torch.float64, device="cuda")
+    e32 = torch.empty(0, dtype=torch.float32, device="cuda")
+    per = dev(np.array([0.5, 0.7]))
+    s, c = gp.gpfc_fold(e64, e32, per, 16)                  # n = 0: zero rows
+    assert not s.cpu().numpy().any() and not c.cpu().numpy().any()
+    s, c = gp.gpfc_fold(e64, e32, e64, 16)                  # nperiods = 0: no-op
+    assert s.shape == (0, 16)
+    with pytest.raises(gp.GpfcError):
+        gp.gpfc_fold(e64, e32, per, 0)
+    with pytest.raises(gp.GpfcError):
+        gp.gpfc_fold(e64, e32, per, 5000)
+    with pytest.raises(gp.GpfcError):
+        gp.gpfc_fold(torch.empty(4, dtype=torch.float64), e32, per, 16)   # host tensor
