@@ -1,0 +1,390 @@
+#!/usr/bin/env python
+"""bench.py -- point-periods folded per second on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (period grid -> phase ->
+bin map -> accumulate -> bin mean -> noise normalisation) over one batch of
+synthetic light curves, through the C ABI of libgpfc.so:
+
+    gpfc_make_period_grid(...)                       -> periods (device)
+    gpfc_fold_batch(..., out_sum, out_count, out_norm)   (fold + fused normalise)
+
+Default workload: BASELINE.json configs[2], the batched Kepler-shaped fold the
+north_star target is quoted on (1,024 curves x 65,000 samples x 20,000 periods,
+nbins = 256).  Inputs are resident in HBM for `value`; `e2e` runs the same step
+through gpfc_fold_batch_host with pinned HOST buffers (copies inside the timed
+region).  One JSON line on stdout (rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+    python -m torch.distributed.run --nproc-per-node N ... bench.py --gpus N ...
+
+N > 1: the path shards by curve with no exchange step; every rank
+folds its own batch of the same shape (weak scaling), no collective on the data
+path; timing is max over ranks.
+--impl reference: the CPU oracle (oracle/), as it stands, on the host cores, on a
+bounded sample of the same workload (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "point-periods folded/sec (samples x trial periods)"
+UNIT = "point-periods/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (0-4)")
+    ap.add_argument("--impl", default="gpfc", choices=["gpfc", "reference"])
+    ap.add_argument("--curves", type=int, default=0, help="debug: override the number of curves")
+    ap.add_argument("--periods", type=int, default=0, help="debug: override the number of periods")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-peaks", action="store_true", help="skip gpfc_measure_peaks")
+    return ap.parse_args()
+
+
+def make_workload(args, rank):
+    from paper_2312_02063_b200 import workloads
+    kw = {}
+    if args.periods:
+        kw["nperiods"] = args.periods
+    if args.config in (2, 4):
+        full = 1024 if args.config == 2 else 4096
+        nc = args.curves or full
+        kw["ncurves"] = nc
+        kw["first_curve"] = rank * nc        # every rank its own curves (weak scaling)
+    return workloads.make(args.config, **kw)
+
+
+def workload_desc(w, args):
+    d = {"workload": "BASELINE.json configs[%d] %s" % (w.config_id, w.name),
+         "curves": w.ncurves, "samples_per_curve": int(w.n_total // max(w.ncurves, 1)),
+         "nperiods": int(w.nperiods), "nbins": int(w.nbins),
+         "outputs": "norm" if w.fused_normalize else "sum+count+norm",
+         "grid": "uniform in frequency, 1/%.1f..1/%.1f d^-1" % (w.pmax, w.pmin),
+         "l2": "inputs + outputs per step exceed the 126 MB L2; no explicit flush"}
+    if args.curves or args.periods:
+        d["reduced"] = True
+    return d
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------- oracle legs
+def oracle_sample(w, periods_host, budget_pp):
+    """Bounded sample of the workload for the CPU oracle: the first curve(s) and the
+    first periods, about `budget_pp` point-periods."""
+    n0 = int(w.offsets[1] - w.offsets[0]) if w.ncurves else 0
+    npd = int(min(w.nperiods, max(1, budget_pp // max(n0, 1))))
+    return 1 if w.ncurves else 0, npd
+
+
+def run_oracle(w, periods_host, ncurves, npd, threads):
+    """Oracle fold + normalise of `ncurves` curves x first `npd` periods, the period axis
+    split over a thread pool (each chunk is the plain single-threaded C routine)."""
+    from concurrent.futures import ThreadPoolExecutor
+    from oracle import ref
+    off = w.offsets[:ncurves + 1]
+    t = w.times[:off[-1]]
+    f = w.flux[:off[-1]]
+    per = np.ascontiguousarray(periods_host[:npd])
+    nchunks = max(1, min(npd, threads))
+    edges = np.linspace(0, npd, nchunks + 1).astype(np.int64)
+
+    def work(i):
+        lo, hi = int(edges[i]), int(edges[i + 1])
+        if hi > lo:
+            ref.fold_batch(t, f, off, per[lo:hi], w.nbins, want_norm=True, want64=False)
+
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        list(ex.map(work, range(nchunks)))
+    dt = time.perf_counter() - t0
+    pp = int(off[-1]) * npd
+    return pp, dt
+
+
+def cpu_baseline(w, periods_host):
+    from oracle import ref
+    ref.build()
+    cores = os.cpu_count() or 1
+    # calibrate on a small slice, then size the sample for ~15 s
+    nc, npd0 = oracle_sample(w, periods_host, 65000 * cores * 2)
+    pp0, dt0 = run_oracle(w, periods_host, nc, npd0, cores)
+    rate0 = pp0 / max(dt0, 1e-9)
+    nc, npd = oracle_sample(w, periods_host, int(rate0 * 15.0))
+    pp, dt = run_oracle(w, periods_host, nc, npd, cores)
+    return {"value": pp / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "curve 0 x first %d periods (%.3g point-periods, %.1f s), fold + normalise, "
+                      "period axis split over %d threads" % (npd, pp, dt, cores)}
+
+
+def reference_arm(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import ref
+    ref.build()
+    w = make_workload(args, 0)
+    periods = ref.make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode)
+    cores = os.cpu_count() or 1
+    nc, npd0 = oracle_sample(w, periods, 65000 * cores)
+    pp0, dt0 = run_oracle(w, periods, nc, npd0, cores)
+    total = max(args.steps + args.warmup, 1)
+    per_step_s = min(20.0, 150.0 / total)
+    nc, npd = oracle_sample(w, periods, int(pp0 / max(dt0, 1e-9) * per_step_s))
+    for _ in range(args.warmup):
+        run_oracle(w, periods, nc, npd, cores)
+    pps, dts = 0, 0.0
+    for _ in range(args.steps):
+        pp, dt = run_oracle(w, periods, nc, npd, cores)
+        pps += pp
+        dts += dt
+    value = pps / max(dts, 1e-12)
+    sample = ("each step: curve 0 x first %d periods (%.3g point-periods), fold + normalise, "
+              "%d threads" % (npd, float(pp), cores))
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+           "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": 1e3 * dts / max(args.steps, 1), "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": workload_desc(w, args),
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                            "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0,
+                   "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+# --------------------------------------------------------------------------- GPU arm
+def gpu_arm(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2312_02063_b200 import binding as gp
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    gp.lib()
+
+    w = make_workload(args, rank)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    times, flux, offsets = dev(w.times), dev(w.flux), dev(w.offsets)
+    shape = (w.ncurves, w.nperiods, w.nbins)
+    periods = torch.empty(w.nperiods, dtype=torch.float64, device="cuda")
+    out_norm = torch.empty(shape, dtype=torch.float32, device="cuda")
+    out_sum = out_count = None
+    if not w.fused_normalize:
+        out_sum = torch.empty(shape, dtype=torch.float32, device="cuda")
+        out_count = torch.empty(shape, dtype=torch.int32, device="cuda")
+    ws = torch.empty(gp.gpfc_workspace_bytes(w.ncurves, w.n_total, w.nperiods, w.nbins),
+                     dtype=torch.uint8, device="cuda")
+    gp.gpfc_set_workspace(ws)
+
+    def step():
+        gp.gpfc_make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode, out=periods)
+        gp.gpfc_fold_batch(times, flux, offsets, periods, w.nbins, out_sum=out_sum,
+                           out_count=out_count, out_norm=out_norm)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    peaks = None
+    if rank == 0 and not args.no_peaks:
+        peaks = gp.gpfc_measure_peaks()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    gp.gpfc_profile(True)
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    prof = gp.gpfc_profile_read()
+    gp.gpfc_profile(False)
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        tt = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    pp_step_all = float(w.point_periods) * world
+    value = pp_step_all * args.steps / (ms * 1e-3)
+
+    # ---- e2e: the same step through the host-buffer entry points (pinned host memory)
+    e2e = None
+    if not args.no_e2e:
+        del out_norm, out_sum, out_count
+        torch.cuda.empty_cache()
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        h_t, h_f, h_o = pin(w.times), pin(w.flux), pin(w.offsets)
+        h_norm = torch.empty(shape, dtype=torch.float32).pin_memory()
+        h_sum = h_cnt = None
+        if not w.fused_normalize:
+            h_sum = torch.empty(shape, dtype=torch.float32).pin_memory()
+            h_cnt = torch.empty(shape, dtype=torch.int32).pin_memory()
+
+        def step_host():
+            per = gp.gpfc_make_period_grid_host(w.pmin, w.pmax, w.nperiods, w.grid_mode)
+            gp.gpfc_fold_batch_host(h_t, h_f, h_o, per, w.nbins, out_sum=h_sum, out_count=h_cnt,
+                                    out_norm=h_norm)
+
+        nwarm = min(args.warmup, 1)
+        nstep = max(1, min(args.steps, 3))
+        for _ in range(nwarm):
+            step_host()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(nstep):
+            step_host()
+        barrier()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt = float(tt.item())
+        nout = int(np.prod(shape)) * 4
+        e2e = {"value": pp_step_all * nstep / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(w.n_total * 12 + w.offsets.nbytes),
+               "d2h_bytes_per_step": int(nout * (1 if w.fused_normalize else 3) + w.nperiods * 8),
+               "steps": nstep, "api": "gpfc_make_period_grid_host + gpfc_fold_batch_host"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the fold kernel), DESIGN.md "Roofline"
+    fold_ms = prof["fold_kernel_ms"] / max(prof["fold_launches"], 1)
+    updates = 2.0 * float(w.point_periods)             # one sum + one count update per point-period
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak_nominal = 148 * 32 * sm_max * 1e6              # 32 shared-memory atomic lanes / clk / SM
+    achieved = updates / (fold_ms * 1e-3)
+    out_bytes = float(np.prod(shape)) * 4 * (1 if w.fused_normalize else 3)
+    roof = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_nominal / 1e9,
+            "unit": "G shared-atomic lane-updates/s", "frac": achieved / peak_nominal,
+            "traffic": None,
+            "kernel": "fold_cols_kernel", "kernel_ms": fold_ms,
+            "peak_source": "derived: 148 SMs x 32 lanes/clk x %.0f MHz" % sm_max,
+            "hbm_bound": {"algorithmic_bytes": out_bytes + w.n_total * 12.0,
+                          "achieved_gbs": (out_bytes + w.n_total * 12.0) / (fold_ms * 1e-3) / 1e9}}
+    try:
+        mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        roof["hbm_bound"]["peak_gbs"] = mp["hbm_gbs"]
+        roof["hbm_bound"]["frac"] = roof["hbm_bound"]["achieved_gbs"] / mp["hbm_gbs"]
+    except (OSError, KeyError, ValueError):
+        roof["hbm_bound"]["peak_gbs"] = 6650.0
+        roof["hbm_bound"]["peak_source"] = "fallback"
+    if peaks:
+        roof["measured_peak"] = peaks["smem_atomic_lane_updates_per_s"] / 1e9
+        roof["frac_of_measured"] = achieved / peaks["smem_atomic_lane_updates_per_s"]
+        roof["fp64_pairs_per_s"] = peaks["fp64_mul_add_pairs_per_s"]
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": workload_desc(w, args), "clocks": clocks, "roofline": roof,
+           "gpu_launches": int(prof["kernel_launches"])}
+    if e2e:
+        out["e2e"] = e2e
+    if not args.no_cpu:
+        periods_host = periods.cpu().numpy()
+        out["cpu_baseline"] = cpu_baseline(w, periods_host)
+    print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        reference_arm(args)
+    else:
+        gpu_arm(args)
+
+
+if __name__ == "__main__":
+    main()

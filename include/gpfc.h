@@ -159,6 +159,17 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
                          float *out_sum, uint32_t *out_count, float *out_norm);
 
 /*
+ * Measurement hooks for bench.py (per calling thread).  gpfc_profile(1) clears the
+ * counters and makes every later fold call record a CUDA-event pair around its
+ * fold-kernel launch on the call's stream; gpfc_profile(0) clears and stops.
+ * gpfc_profile_read waits for the recorded events and returns the summed
+ * fold-kernel time (ms), the number of fold-kernel launches timed, and the number
+ * of kernels of this library launched since gpfc_profile() (any may be NULL).
+ */
+int gpfc_profile(int enable);
+int gpfc_profile_read(double *fold_kernel_ms, int64_t *fold_launches, int64_t *kernel_launches);
+
+/*
  * Roofline calibration: runs the library's micro-kernels on
  * the current stream and reports the measured peak rates of the units that
  * bound the fold, so that bench.py can quote its denominator from the same run

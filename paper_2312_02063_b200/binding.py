@@ -27,7 +27,7 @@ EXPORTS = [
     "gpfc_version", "gpfc_last_error", "gpfc_set_stream", "gpfc_workspace_bytes",
     "gpfc_set_workspace", "gpfc_make_period_grid", "gpfc_n_sample", "gpfc_fold",
     "gpfc_normalize", "gpfc_fold_batch", "gpfc_make_period_grid_host",
-    "gpfc_fold_batch_host", "gpfc_measure_peaks",
+    "gpfc_fold_batch_host", "gpfc_measure_peaks", "gpfc_profile", "gpfc_profile_read",
 ]
 
 
@@ -64,6 +64,8 @@ def lib() -> ctypes.CDLL:
     L.gpfc_fold_batch.argtypes = fb
     L.gpfc_fold_batch_host.argtypes = fb
     L.gpfc_measure_peaks.argtypes = [vp]
+    L.gpfc_profile.argtypes = [i32]
+    L.gpfc_profile_read.argtypes = [vp, vp, vp]
     _lib = L
     return L
 
@@ -214,3 +216,16 @@ def gpfc_measure_peaks() -> dict:
     _check(lib().gpfc_measure_peaks(out), "gpfc_measure_peaks")
     return {"smem_atomic_lane_updates_per_s": out[0], "fp64_mul_add_pairs_per_s": out[1],
             "fold_loop_pp_per_s": out[2]}
+
+
+def gpfc_profile(enable: bool) -> None:
+    _check(lib().gpfc_profile(1 if enable else 0), "gpfc_profile")
+
+
+def gpfc_profile_read() -> dict:
+    ms = ctypes.c_double(0.0)
+    nf = ctypes.c_int64(0)
+    nk = ctypes.c_int64(0)
+    _check(lib().gpfc_profile_read(ctypes.byref(ms), ctypes.byref(nf), ctypes.byref(nk)),
+           "gpfc_profile_read")
+    return {"fold_kernel_ms": ms.value, "fold_launches": nf.value, "kernel_launches": nk.value}

@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <vector>
 
 #include "common.cuh"
 
@@ -13,6 +14,10 @@ struct ThreadState {
     void *ws = nullptr;
     size_t ws_bytes = 0;
     char err[512] = "";
+    // gpfc_profile: CUDA-event pairs around every fold-kernel launch + launch counter
+    bool profiling = false;
+    long long launches = 0;
+    std::vector<cudaEvent_t> ev;      // start, stop, start, stop, ...
 };
 
 thread_local ThreadState g_ts;
@@ -95,7 +100,9 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
     if (!offsets) {   // single-curve entry point
         set_offsets_kernel<<<1, 1, 0, st>>>(own_off, n_total);
         offsets = own_off;
+        g_ts.launches += 1;
     }
+    g_ts.launches += 3;   // prep_curves, prep_periods, fold
     e = gpfc::launch_prep(times, flux, offsets, ncurves, t0v, t0_scalar, periods, nperiods, nbins,
                           s, st);
     if (e == cudaSuccess) {
@@ -111,7 +118,16 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
         a.out_sum = out_sum;
         a.out_count = out_count;
         a.out_norm = out_norm;
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        if (g_ts.profiling && cudaEventCreate(&e0) == cudaSuccess &&
+            cudaEventCreate(&e1) == cudaSuccess)
+            cudaEventRecord(e0, st);
         e = gpfc::launch_fold(a, st);
+        if (e0 && e1) {
+            cudaEventRecord(e1, st);
+            g_ts.ev.push_back(e0);
+            g_ts.ev.push_back(e1);
+        }
     }
     if (own) {
         cudaError_t e2 = cudaFreeAsync(base, st);
@@ -170,6 +186,7 @@ int gpfc_make_period_grid(double pmin, double pmax, int64_t nperiods, int mode_f
     if (!periods_out) return fail(GPFC_ERR_INVALID_ARG, "periods_out is NULL%s");
     cudaError_t e = gpfc::launch_grid(pmin, pmax, nperiods, mode_flags, periods_out, g_ts.stream);
     if (e != cudaSuccess) return cuda_fail(e, "grid launch");
+    g_ts.launches += 1;
     return GPFC_OK;
 }
 
@@ -191,6 +208,7 @@ int gpfc_normalize(const float *sum, const uint32_t *count, int64_t nprofiles, i
     if (!sum || !count || !out_norm) return fail(GPFC_ERR_INVALID_ARG, "NULL pointer%s");
     cudaError_t e = gpfc::launch_normalize(sum, count, nprofiles, nbins, out_norm, g_ts.stream);
     if (e != cudaSuccess) return cuda_fail(e, "normalize launch");
+    g_ts.launches += 1;
     return GPFC_OK;
 }
 
@@ -216,6 +234,7 @@ int gpfc_make_period_grid_host(double pmin, double pmax, int64_t nperiods, int m
     cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&d), (size_t)nperiods * 8, st);
     if (e != cudaSuccess) return cuda_fail(e, "grid alloc");
     e = gpfc::launch_grid(pmin, pmax, nperiods, mode_flags, d, st);
+    g_ts.launches += 1;
     if (e == cudaSuccess)
         e = cudaMemcpyAsync(periods_out, d, (size_t)nperiods * 8, cudaMemcpyDeviceToHost, st);
     cudaFreeAsync(d, st);
@@ -292,6 +311,31 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
     if (rc != GPFC_OK) return rc;
     if (e == cudaSuccess) e = e2;
     if (e != cudaSuccess) return cuda_fail(e, "host-buffer fold");
+    return GPFC_OK;
+}
+
+int gpfc_profile(int enable)
+{
+    for (cudaEvent_t ev : g_ts.ev) cudaEventDestroy(ev);
+    g_ts.ev.clear();
+    g_ts.launches = 0;
+    g_ts.profiling = enable != 0;
+    return GPFC_OK;
+}
+
+int gpfc_profile_read(double *fold_kernel_ms, int64_t *fold_launches, int64_t *kernel_launches)
+{
+    double total = 0.0;
+    for (size_t i = 0; i + 1 < g_ts.ev.size(); i += 2) {
+        cudaError_t e = cudaEventSynchronize(g_ts.ev[i + 1]);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, g_ts.ev[i], g_ts.ev[i + 1]);
+        if (e != cudaSuccess) return cuda_fail(e, "gpfc_profile_read");
+        total += ms;
+    }
+    if (fold_kernel_ms) *fold_kernel_ms = total;
+    if (fold_launches) *fold_launches = (int64_t)(g_ts.ev.size() / 2);
+    if (kernel_launches) *kernel_launches = g_ts.launches;
     return GPFC_OK;
 }
 
