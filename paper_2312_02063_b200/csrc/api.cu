@@ -41,6 +41,8 @@ size_t scratch_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods)
     size_t b = 0;
     b += align_up((size_t)n_total * sizeof(double));
     b += align_up((size_t)n_total * sizeof(int));
+    b += align_up((size_t)n_total * sizeof(int4));
+    b += align_up(((size_t)n_total / gpfc::GPFC_TILE + (size_t)ncurves + 1) * sizeof(gpfc::TileInfo));
     b += align_up((size_t)ncurves * sizeof(gpfc::CurveMeta));
     b += align_up((size_t)nperiods * sizeof(double));
     b += align_up(2 * sizeof(int64_t));   // offsets of the single-curve call
@@ -90,6 +92,10 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
     cur += align_up((size_t)n_total * sizeof(double));
     s.q = reinterpret_cast<int *>(cur);
     cur += align_up((size_t)n_total * sizeof(int));
+    s.rec = reinterpret_cast<int4 *>(cur);
+    cur += align_up((size_t)n_total * sizeof(int4));
+    s.tiles = reinterpret_cast<gpfc::TileInfo *>(cur);
+    cur += align_up(((size_t)n_total / gpfc::GPFC_TILE + (size_t)ncurves + 1) * sizeof(gpfc::TileInfo));
     s.meta = reinterpret_cast<gpfc::CurveMeta *>(cur);
     cur += align_up((size_t)ncurves * sizeof(gpfc::CurveMeta));
     s.rp = reinterpret_cast<double *>(cur);
@@ -109,6 +115,8 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
         gpfc::FoldArgs a;
         a.u = s.u;
         a.q = s.q;
+        a.rec = s.rec;
+        a.tiles = s.tiles;
         a.meta = s.meta;
         a.rp = s.rp;
         a.periods = periods;

@@ -9,28 +9,45 @@
 
 namespace gpfc {
 
+// Samples are handled in anchor tiles of GPFC_TILE consecutive (compacted) samples of a
+// curve: the prepass stores, per tile, the smallest u (the anchor a) and the tile's span,
+// and per sample the 16-byte record {v = u - a (fp64), q (int32), 0}.
+constexpr int GPFC_TILE = 128;
+
+struct TileInfo {
+    double a;      // min of u over the tile
+    double span;   // max - min of u over the tile
+};
+
 // Per-curve table written by the prepass (prep.cu) and read by the fold.
 struct CurveMeta {
-    long long start;   // first compacted sample of this curve in the u / q scratch arrays
+    long long start;   // first compacted sample of this curve in the u / q / rec scratch arrays
+    long long tile0;   // first entry of this curve in the tile table
     int n_valid;       // samples with finite time and flux (compacted to the front)
     int shift;         // fixed-point exponent s: q = rint((flux - center) * 2^s)
     double center;     // per-curve constant removed before quantisation (0 for centred input)
     double inv_scale;  // 2^-s
     double umin;       // min / max of u = t - t0 over the valid samples
     double umax;
+    double span_max;   // largest tile span of the curve
 };
 
 // Scratch carved out of the workspace for one gpfc_fold_batch call.
 struct Scratch {
     double *u;         // [n_total]  t - t0, valid samples compacted per curve
     int *q;            // [n_total]  fixed-point flux
+    int4 *rec;         // [n_total]  {lo(v), hi(v), q, 0}, v = u - anchor of the sample's tile
+    TileInfo *tiles;   // [n_total / GPFC_TILE + ncurves + 1]
     CurveMeta *meta;   // [ncurves]
-    double *rp;        // [nperiods] RN(1/P) * nbins, NaN for a period that is not finite-positive
+    double *rp;        // [nperiods] RN(1/P) * rows, NaN for a period that is not finite-positive;
+                       // rows = 256 for power-of-two nbins in [32, 256] (lane-period kernel), else nbins
 };
 
 struct FoldArgs {
     const double *u;
     const int *q;
+    const int4 *rec;
+    const TileInfo *tiles;
     const CurveMeta *meta;
     const double *rp;
     const double *periods;
@@ -143,6 +160,9 @@ cudaError_t launch_prep(const double *times, const float *flux, const int64_t *o
                         const double *periods, long long nperiods, int nbins, Scratch s,
                         cudaStream_t st);
 cudaError_t launch_fold(const FoldArgs &a, cudaStream_t st);
+cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st);   // fold_lp.cu: nbins in {32,64,128,256}
+bool fold_lp_handles(int nbins);
+int num_sms();
 cudaError_t launch_normalize(const float *sum, const uint32_t *count, long long nprofiles,
                              int nbins, float *out, cudaStream_t st);
 cudaError_t launch_grid(double pmin, double pmax, long long nperiods, int mode_flags,

@@ -277,21 +277,6 @@ fold_generic_kernel(FoldArgs a, long long nitems)
     }
 }
 
-int g_num_sms = 0;
-
-int num_sms()
-{
-    if (g_num_sms == 0) {
-        int dev = 0, n = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
-            g_num_sms = n;
-        else
-            return 148;
-    }
-    return g_num_sms;
-}
-
 template <int NBLOG, int COLSLOG, int PB, int KS>
 cudaError_t launch_cols(const FoldArgs &a, cudaStream_t st)
 {
@@ -313,14 +298,25 @@ cudaError_t launch_cols(const FoldArgs &a, cudaStream_t st)
 
 }  // namespace
 
+int num_sms()
+{
+    static int g_num_sms = 0;
+    if (g_num_sms == 0) {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+            g_num_sms = n;
+        else
+            return 148;
+    }
+    return g_num_sms;
+}
+
 cudaError_t launch_fold(const FoldArgs &a, cudaStream_t st)
 {
     if (a.ncurves <= 0 || a.nperiods <= 0) return cudaSuccess;
+    if (fold_lp_handles(a.nbins)) return launch_fold_lp(a, st);
     switch (a.nbins) {
-        case 32: return launch_cols<5, 5, 8, 4>(a, st);
-        case 64: return launch_cols<6, 5, 8, 4>(a, st);
-        case 128: return launch_cols<7, 5, 6, 4>(a, st);
-        case 256: return launch_cols<8, 5, 3, 4>(a, st);
         case 512: return launch_cols<9, 5, 1, 4>(a, st);
         case 1024: return launch_cols<10, 4, 1, 4>(a, st);
         case 2048: return launch_cols<11, 3, 1, 4>(a, st);

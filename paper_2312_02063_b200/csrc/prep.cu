@@ -62,6 +62,7 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
     __shared__ BlockRed red;
     __shared__ int warp_tot[32];
     __shared__ int tile_base;
+    __shared__ double warp_span[32];
     const long long c = blockIdx.x;
     const long long start = offsets[c];
     const long long n = offsets[c + 1] - start;
@@ -152,9 +153,53 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
         if (tid == PREP_THREADS - 1) tile_base = base + wbase + __popc(bal);
         __syncthreads();
     }
+    // pass 4: anchor tiles of GPFC_TILE compacted samples: anchor a = min u of the tile,
+    // record {v = u - a, q}.  (The compacted u / q were written by this CTA above.)
+    const int n_valid = tile_base;
+    const long long tile0 = start / GPFC_TILE + c;   // disjoint per curve: ceil(n/T) <= n/T + 1
+    double span_max = 0.0;
+    for (int t = warp; t * GPFC_TILE < n_valid; t += PREP_THREADS / 32) {
+        const int base = t * GPFC_TILE;
+        double uu[GPFC_TILE / 32];
+        double lo = CUDART_INF, hi = -CUDART_INF;
+#pragma unroll
+        for (int k = 0; k < GPFC_TILE / 32; ++k) {
+            int i = base + k * 32 + lane;
+            uu[k] = (i < n_valid) ? s.u[start + i] : CUDART_NAN;
+            if (i < n_valid) {
+                lo = fmin(lo, uu[k]);
+                hi = fmax(hi, uu[k]);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+            hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        }
+#pragma unroll
+        for (int k = 0; k < GPFC_TILE / 32; ++k) {
+            int i = base + k * 32 + lane;
+            if (i < n_valid) {
+                double v = __dsub_rn(uu[k], lo);
+                s.rec[start + i] = make_int4(__double2loint(v), __double2hiint(v), s.q[start + i], 0);
+            }
+        }
+        if (lane == 0) {
+            TileInfo ti;
+            ti.a = lo;
+            ti.span = __dsub_ru(hi, lo);
+            s.tiles[tile0 + t] = ti;
+        }
+        span_max = fmax(span_max, __dsub_ru(hi, lo));
+    }
+    if (lane == 0) warp_span[warp] = span_max;
+    __syncthreads();
     if (tid == 0) {
+        for (int w = 0; w < PREP_THREADS / 32; ++w) span_max = fmax(span_max, warp_span[w]);
         CurveMeta m;
         m.start = start;
+        m.tile0 = tile0;
+        m.span_max = span_max;
         m.n_valid = tile_base;
         m.shift = shift;
         m.center = center;
@@ -165,8 +210,9 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
     }
 }
 
-// rp[j] = RN(1/P_j) * nbins (exact scaling for power-of-two nbins), NaN when the
-// period is not finite and positive.
+// rp[j] = RN(1/P_j) * rows (exact scaling for power-of-two rows), NaN when the
+// period is not finite and positive.  rows = nbins, or 256 when the lane-period kernel
+// folds at 256 rows and merges adjacent rows at write-out (fold_lp.cu).
 __global__ void prep_periods_kernel(const double *__restrict__ periods, long long nperiods,
                                     int nbins, double *__restrict__ rp)
 {
@@ -190,7 +236,8 @@ cudaError_t launch_prep(const double *times, const float *flux, const int64_t *o
                                                                       t0_scalar, s);
     if (nperiods > 0) {
         unsigned blocks = (unsigned)((nperiods + 255) / 256);
-        prep_periods_kernel<<<blocks, 256, 0, st>>>(periods, nperiods, nbins, s.rp);
+        prep_periods_kernel<<<blocks, 256, 0, st>>>(periods, nperiods,
+                                                    fold_lp_handles(nbins) ? 256 : nbins, s.rp);
     }
     return cudaGetLastError();
 }
