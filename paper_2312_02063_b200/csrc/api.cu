@@ -41,7 +41,7 @@ size_t scratch_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods)
     size_t b = 0;
     b += align_up((size_t)n_total * sizeof(double));
     b += align_up((size_t)n_total * sizeof(int));
-    b += align_up((size_t)n_total * sizeof(int4));
+    b += align_up(((size_t)n_total + (size_t)ncurves + 2) * sizeof(int2));
     b += align_up(((size_t)n_total / gpfc::GPFC_TILE + (size_t)ncurves + 1) * sizeof(gpfc::TileInfo));
     b += align_up((size_t)ncurves * sizeof(gpfc::CurveMeta));
     b += align_up((size_t)nperiods * sizeof(double));
@@ -92,8 +92,8 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
     cur += align_up((size_t)n_total * sizeof(double));
     s.q = reinterpret_cast<int *>(cur);
     cur += align_up((size_t)n_total * sizeof(int));
-    s.rec = reinterpret_cast<int4 *>(cur);
-    cur += align_up((size_t)n_total * sizeof(int4));
+    s.rec = reinterpret_cast<int2 *>(cur);
+    cur += align_up(((size_t)n_total + (size_t)ncurves + 2) * sizeof(int2));
     s.tiles = reinterpret_cast<gpfc::TileInfo *>(cur);
     cur += align_up(((size_t)n_total / gpfc::GPFC_TILE + (size_t)ncurves + 1) * sizeof(gpfc::TileInfo));
     s.meta = reinterpret_cast<gpfc::CurveMeta *>(cur);

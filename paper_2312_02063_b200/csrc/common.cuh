@@ -10,18 +10,20 @@
 namespace gpfc {
 
 // Samples are handled in anchor tiles of GPFC_TILE consecutive (compacted) samples of a
-// curve: the prepass stores, per tile, the smallest u (the anchor a) and the tile's span,
-// and per sample the 16-byte record {v = u - a (fp64), q (int32), 0}.
+// curve: the prepass stores, per tile, the smallest u (the anchor a) and a power-of-two
+// scale 2^-S with (max u - a) * 2^S < 2^32, and per sample the 8-byte record
+// {iv = rint((u - a) * 2^S) (uint32), q (int32)}: |iv * 2^-S - (u - a)| <= 2^-S.
 constexpr int GPFC_TILE = 128;
 
 struct TileInfo {
-    double a;      // min of u over the tile
-    double span;   // max - min of u over the tile
+    double a;          // min of u over the tile
+    double inv_scale;  // 2^-S
 };
 
 // Per-curve table written by the prepass (prep.cu) and read by the fold.
 struct CurveMeta {
-    long long start;   // first compacted sample of this curve in the u / q / rec scratch arrays
+    long long start;   // first compacted sample of this curve in the u / q scratch arrays
+    long long rec0;    // first record of this curve in rec (even: 16-byte aligned)
     long long tile0;   // first entry of this curve in the tile table
     int n_valid;       // samples with finite time and flux (compacted to the front)
     int shift;         // fixed-point exponent s: q = rint((flux - center) * 2^s)
@@ -30,13 +32,14 @@ struct CurveMeta {
     double umin;       // min / max of u = t - t0 over the valid samples
     double umax;
     double span_max;   // largest tile span of the curve
+    double pivot;      // mean of the centred, quantised flux: (sum q) 2^-s / n_valid
 };
 
 // Scratch carved out of the workspace for one gpfc_fold_batch call.
 struct Scratch {
     double *u;         // [n_total]  t - t0, valid samples compacted per curve
     int *q;            // [n_total]  fixed-point flux
-    int4 *rec;         // [n_total]  {lo(v), hi(v), q, 0}, v = u - anchor of the sample's tile
+    int2 *rec;         // [n_total + ncurves + 2]  {iv, q} (see GPFC_TILE)
     TileInfo *tiles;   // [n_total / GPFC_TILE + ncurves + 1]
     CurveMeta *meta;   // [ncurves]
     double *rp;        // [nperiods] RN(1/P) * rows, NaN for a period that is not finite-positive;
@@ -46,7 +49,7 @@ struct Scratch {
 struct FoldArgs {
     const double *u;
     const int *q;
-    const int4 *rec;
+    const int2 *rec;
     const TileInfo *tiles;
     const CurveMeta *meta;
     const double *rp;

@@ -10,10 +10,11 @@
 //   (bank = lane), so every ATOMS is one conflict-free wavefront; the atomics only
 //   arbitrate between warps.  No replication, hence no column reduction afterwards, and
 //   32*R periods share every sample load.  No global atomics anywhere.
-// * Samples are staged per warp in shared memory with coalesced 16-byte loads and read
-//   back with one broadcast LDS.128 per sample {v, q}.
+// * Samples are 8-byte records {iv, q} (iv = the sample's offset from its tile anchor in
+//   32-bit fixed point), staged per warp in shared memory with coalesced 16-byte loads and
+//   read back with one broadcast LDS.128 per TWO samples; one I2F.F64 per sample.
 // * Phase math per point-period is ONE fp64 instruction: m = RD(v * rp + C) (DFMA.RM),
-//   v = u - a the sample's offset from its tile anchor, rp = 256 * RN(1/P),
+//   v = iv 2^-S ~ u - a, rp = 256 * RN(1/P),
 //   C = 2^20 + delta + ((a * rp) mod 256) set up once per (tile, period).  ulp(m) = 2^-32:
 //   the low word of m is the fraction of the row coordinate, bits 0..7 of the high word
 //   are the row.  One PRMT builds the shared-memory address (row * 256 + lane * 4), one
@@ -39,21 +40,22 @@ constexpr int LP_R = 3;                       // periods per lane
 constexpr int LP_GROUP = 32 * LP_R;           // periods per work item
 constexpr int LP_ROWS = 256;                  // rows per period (fold resolution)
 constexpr int LP_GRAN = 64;                   // samples per staging granule
-constexpr int LP_PARTS = 4;                   // bin ranges per period in the statistics sweeps
 constexpr unsigned LP_SMEM_BASE = 0x400;      // shared-window address of dynamic shared memory
 
 constexpr int LP_HIST_BYTES = LP_R * LP_ROWS * 256;           // 196,608
-constexpr int LP_STAGE_OFF = LP_HIST_BYTES;                   // int4 [LP_WARPS][LP_GRAN]
-constexpr int LP_STAGE_BYTES = LP_WARPS * LP_GRAN * 16;
-constexpr int LP_PART_OFF = LP_STAGE_OFF + LP_STAGE_BYTES;    // double [LP_PARTS][LP_GROUP]
-constexpr int LP_PARTK_OFF = LP_PART_OFF + LP_PARTS * LP_GROUP * 8;   // int [LP_PARTS][LP_GROUP]
-constexpr int LP_MU_OFF = LP_PARTK_OFF + LP_PARTS * LP_GROUP * 4;     // double [LP_GROUP]
+// scratch after the histograms: sample staging during the fold, statistics partials in the
+// epilogue (the two never live at the same time)
+constexpr int LP_STAGE_OFF = LP_HIST_BYTES;                   // int2 [LP_WARPS][LP_GRAN]
+constexpr int LP_PS1_OFF = LP_HIST_BYTES;                     // double [LP_WARPS][LP_GROUP]
+constexpr int LP_PS2_OFF = LP_PS1_OFF + LP_WARPS * LP_GROUP * 8;
+constexpr int LP_PKK_OFF = LP_PS2_OFF + LP_WARPS * LP_GROUP * 8;      // int [LP_WARPS][LP_GROUP]
+constexpr int LP_MU_OFF = LP_PKK_OFF + LP_WARPS * LP_GROUP * 4;       // double [LP_GROUP]
 constexpr int LP_ISD_OFF = LP_MU_OFF + LP_GROUP * 8;                  // double [LP_GROUP]
 constexpr int LP_KK_OFF = LP_ISD_OFF + LP_GROUP * 8;                  // int [LP_GROUP]
 constexpr int LP_CTR_OFF = LP_KK_OFF + LP_GROUP * 4;
 constexpr int LP_SMEM_BYTES = LP_CTR_OFF + 16;
 static_assert(LP_SMEM_BYTES <= 227 * 1024, "shared memory budget");
-static_assert(LP_R * LP_PARTS <= LP_WARPS, "statistics sweep needs R * PARTS warps");
+static_assert(LP_WARPS * LP_GRAN * 8 <= LP_MU_OFF - LP_STAGE_OFF, "staging fits in the scratch");
 
 // shared-memory reductions with an immediate offset: ATOMS.ADD / ATOMS.POPC.INC
 template <int IMM>
@@ -90,16 +92,17 @@ template <int r0>
 struct ForR {
     __device__ __forceinline__ static void run(double v, int q, const double (&rp)[LP_R],
                                                const double (&C)[LP_R], unsigned lane4,
-                                               unsigned &gmin)
+                                               unsigned (&gmin)[LP_R])
     {
-        pp_update<r0>(v, q, rp[r0], C[r0], lane4, gmin);
+        pp_update<r0>(v, q, rp[r0], C[r0], lane4, gmin[r0]);
         ForR<r0 + 1>::run(v, q, rp, C, lane4, gmin);
     }
 };
 template <>
 struct ForR<LP_R> {
     __device__ __forceinline__ static void run(double, int, const double (&)[LP_R],
-                                               const double (&)[LP_R], unsigned, unsigned &) {}
+                                               const double (&)[LP_R], unsigned,
+                                               unsigned (&)[LP_R]) {}
 };
 
 __global__ void __launch_bounds__(LP_THREADS, 1)
@@ -111,9 +114,9 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
         return;
     }
     unsigned *H = reinterpret_cast<unsigned *>(smem);
-    int4 *stage_all = reinterpret_cast<int4 *>(smem + LP_STAGE_OFF);
-    double *part_s = reinterpret_cast<double *>(smem + LP_PART_OFF);
-    int *part_k = reinterpret_cast<int *>(smem + LP_PARTK_OFF);
+    double *ps1 = reinterpret_cast<double *>(smem + LP_PS1_OFF);
+    double *ps2 = reinterpret_cast<double *>(smem + LP_PS2_OFF);
+    int *pkk = reinterpret_cast<int *>(smem + LP_PKK_OFF);
     double *st_mu = reinterpret_cast<double *>(smem + LP_MU_OFF);
     double *st_isd = reinterpret_cast<double *>(smem + LP_ISD_OFF);
     int *st_kk = reinterpret_cast<int *>(smem + LP_KK_OFF);
@@ -121,7 +124,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned lane4 = (unsigned)lane << 2;
-    int4 *stage = stage_all + warp * LP_GRAN;
+    int4 *stage = reinterpret_cast<int4 *>(smem + LP_STAGE_OFF) + warp * (LP_GRAN / 2);
     for (int i = tid; i < LP_HIST_BYTES / 4; i += LP_THREADS) H[i] = 0u;
     if (tid == 0) *ctr = 0;
     __syncthreads();
@@ -130,6 +133,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
     const int mshift = 8 - (31 - __clz(nb));     // rows merged per bin = 1 << mshift
     const int M = 1 << mshift;
     const double M2 = 1729382256910270464.0;     // 1.5 * 2^60: ulp = 256
+    const bool want_norm = a.out_norm != nullptr;
 
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const long long curve = item / ngroups;
@@ -153,15 +157,16 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) rpmax = fmax(rpmax, __shfl_xor_sync(0xffffffffu, rpmax, o));
 
-        // guard band, in units of 2^-32 row:
-        //   E <= 4 * 2^-53 * max|u| * rpmax + 2^-33 + 2^-46  ->  eunits = 4 U rpmax 2^-21 + 1
-        //   delta >= E + 1 unit, D = 2 delta  ->  D >= 2 eunits + 2
+        // guard band, in units of 2^-32 row.  Per item:
+        //   ebase = 4 * 2^-53 * max|u| * rpmax * 2^32 + 1     (roundings of u/P, 1/P, v, C)
+        // per tile, the quantisation of v adds  eq = 2^-S * rpmax * 2^32;
+        //   delta >= E + 1 unit, D = 2 delta  ->  D >= 2 (ebase + eq) + 2
         const double U = fmax(fabs(cm.umin), fabs(cm.umax));
-        const double need = 2.0 * (4.0 * U * rpmax * (1.0 / 2097152.0) + 1.0) + 2.0;
-        unsigned D = 16u;
-        while ((double)D < need && D < 32768u) D <<= 1;
-        const bool fast = (need <= 16384.0) && (cm.span_max * rpmax + 512.0 < 1048576.0);
-        const double K = 1048576.0 + (double)(D >> 1) * (1.0 / 4294967296.0);
+        const double ebase = 4.0 * U * rpmax * (1.0 / 2097152.0) + 1.0;
+        // worst tile of the curve: 2^-S <= 2 span_max 2^-32 (or 2^-40)
+        const double eq_max = fmax(2.0 * cm.span_max, 1.0 / 256.0) * rpmax;
+        const bool fast = (2.0 * (ebase + eq_max) + 2.0 <= 1048576.0) &&
+                          (cm.span_max * rpmax + 512.0 < 1048576.0);
 
         if (fast) {
             for (;;) {
@@ -172,69 +177,76 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 const int base = t * GPFC_TILE;
                 const int cnt = min(GPFC_TILE, n - base);
                 const TileInfo ti = a.tiles[cm.tile0 + t];
-                double C[LP_R];
+                // D = smallest power of two >= need (>= 16): exponent trick, need = f 2^e, f < 1
+                const double need = 2.0 * (ebase + ti.inv_scale * rpmax * 4294967296.0) + 2.0;
+                int ex = ((__double2hiint(need) >> 20) & 0x7ff) - 1022;
+                if (ex < 4) ex = 4;
+                const unsigned D = 1u << ex;
+                const double K = 1048576.0 + (double)(D >> 1) * (1.0 / 4294967296.0);
+                double C[LP_R], rps[LP_R];
 #pragma unroll
                 for (int r = 0; r < LP_R; ++r) {
                     double w = __fma_rd(ti.a, rp[r], M2);       // M2 + 256 * floor(a rp / 256)
                     double z = __dsub_rn(w, M2);
                     double c1 = __fma_rn(ti.a, rp[r], -z);      // (a rp) mod 256, error <= 2^-46
                     C[r] = __dadd_rn(c1, K);
+                    rps[r] = __dmul_rn(rp[r], ti.inv_scale);    // exact (power of two)
                 }
-                const int4 *src = a.rec + cm.start + base;
-                unsigned gmin = 0xffffffffu;
-                int4 n0 = make_int4(0, 0, 0, 0), n1 = n0;
-                if (lane < cnt) n0 = __ldg(src + lane);
-                if (lane + 32 < cnt) n1 = __ldg(src + lane + 32);
+                const int2 *src = a.rec + cm.rec0 + base;      // 16-byte aligned
+                const int4 *src4 = reinterpret_cast<const int4 *>(src);
+                unsigned gmin[LP_R];
+#pragma unroll
+                for (int r = 0; r < LP_R; ++r) gmin[r] = 0xffffffffu;
+                int4 nx = make_int4(0, 0, 0, 0);
+                if (2 * lane < cnt) nx = __ldg(src4 + lane);
                 for (int g0 = 0; g0 < cnt; g0 += LP_GRAN) {
                     const int gc = min(LP_GRAN, cnt - g0);
                     __syncwarp();
-                    stage[lane] = n0;
-                    stage[lane + 32] = n1;
+                    stage[lane] = nx;
                     __syncwarp();
-                    if (g0 + LP_GRAN + lane < cnt) n0 = __ldg(src + g0 + LP_GRAN + lane);
-                    if (g0 + LP_GRAN + lane + 32 < cnt) n1 = __ldg(src + g0 + LP_GRAN + lane + 32);
+                    if (g0 + LP_GRAN + 2 * lane < cnt) nx = __ldg(src4 + (g0 + LP_GRAN) / 2 + lane);
                     if (gc == LP_GRAN) {
 #pragma unroll 1
-                        for (int s = 0; s < LP_GRAN; s += 4) {
-                            int4 rc[4];
-#pragma unroll
-                            for (int k = 0; k < 4; ++k) rc[k] = stage[s + k];
-#pragma unroll
-                            for (int k = 0; k < 4; ++k)
-                                ForR<0>::run(__hiloint2double(rc[k].y, rc[k].x), rc[k].z, rp, C,
-                                             lane4, gmin);
+                        for (int s = 0; s < LP_GRAN / 2; s += 2) {
+                            const int4 ra = stage[s], rb = stage[s + 1];
+                            ForR<0>::run((double)(unsigned)ra.x, ra.y, rps, C, lane4, gmin);
+                            ForR<0>::run((double)(unsigned)ra.z, ra.w, rps, C, lane4, gmin);
+                            ForR<0>::run((double)(unsigned)rb.x, rb.y, rps, C, lane4, gmin);
+                            ForR<0>::run((double)(unsigned)rb.z, rb.w, rps, C, lane4, gmin);
                         }
                     } else {
+                        const int2 *st2 = reinterpret_cast<const int2 *>(stage);
 #pragma unroll 1
                         for (int s = 0; s < gc; ++s) {
-                            int4 rc = stage[s];
-                            ForR<0>::run(__hiloint2double(rc.y, rc.x), rc.z, rp, C, lane4, gmin);
+                            const int2 rc = st2[s];
+                            ForR<0>::run((double)(unsigned)rc.x, rc.y, rps, C, lane4, gmin);
                         }
                     }
                 }
-                if (__any_sync(0xffffffffu, gmin < D)) {
+                unsigned gall = gmin[0];
+#pragma unroll
+                for (int r = 1; r < LP_R; ++r) gall = min(gall, gmin[r]);
+                if (__any_sync(0xffffffffu, gall < D)) {
                     // rare: some row coordinate sat within the guard band of an integer.
                     // Re-check those samples against the exact formula; move the ones that
                     // the fast path put in the wrong row.
-                    if (gmin < D) {
-                        const double *us = a.u + cm.start + base;
+                    const double *us = a.u + cm.start + base;
 #pragma unroll
-                        for (int r = 0; r < LP_R; ++r) {
-                            if (!valid[r]) continue;
-                            const double per = a.periods[p0 + r * 32 + lane];
+                    for (int r = 0; r < LP_R; ++r) {
+                        if (gmin[r] >= D || !valid[r]) continue;
+                        const double per = a.periods[p0 + r * 32 + lane];
 #pragma unroll 1
-                            for (int s = 0; s < cnt; ++s) {
-                                int4 rc = __ldg(src + s);
-                                double m = __fma_rd(__hiloint2double(rc.y, rc.x), rp[r], C[r]);
-                                if ((unsigned)__double2loint(m) < D) {
-                                    int kf = __double2hiint(m) & (LP_ROWS - 1);
-                                    int ke = exact_bin(us[s], per, LP_ROWS);
-                                    if (ke != kf) {
-                                        atomicAdd(&H[hidx(r, kf, 0, lane)], (unsigned)(-rc.z));
-                                        atomicSub(&H[hidx(r, kf, 1, lane)], 1u);
-                                        atomicAdd(&H[hidx(r, ke, 0, lane)], (unsigned)rc.z);
-                                        atomicAdd(&H[hidx(r, ke, 1, lane)], 1u);
-                                    }
+                        for (int s = 0; s < cnt; ++s) {
+                            const int2 rc = __ldg(src + s);
+                            double m = __fma_rd((double)(unsigned)rc.x, rps[r], C[r]);
+                            if ((unsigned)__double2loint(m) < D) {
+                                int kf = __double2hiint(m) & (LP_ROWS - 1);
+                                int ke = exact_bin(us[s], per, LP_ROWS);
+                                if (ke != kf) {
+                                    atomicAdd(&H[hidx(r, kf, 0, lane)], (unsigned)(-rc.y));
+                                    atomicSub(&H[hidx(r, kf, 1, lane)], 1u);
+                                    atomicAdd(&H[hidx(r, ke, 0, lane)], (unsigned)rc.y);
+                                    atomicAdd(&H[hidx(r, ke, 1, lane)], 1u);
                                 }
                             }
                         }
@@ -274,129 +286,138 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
         __syncthreads();   // A: every update of this item is in H
 
         // ---- epilogue.  Lane l reads only its own columns: conflict-free, no cross-lane
-        // reduction.  Bin b = rows b*M .. b*M + M-1.
-        const double inv_scale = cm.inv_scale, center = cm.center;
-        if (a.out_norm) {
-            // sweep 1: number of non-empty bins and sum of bin means (of the centred flux)
-            const int r = warp / LP_PARTS, part = warp % LP_PARTS;
-            const int nbp = nb / LP_PARTS;
-            if (warp < LP_R * LP_PARTS) {
-                double s1 = 0.0;
-                int kk = 0;
-                for (int b = part * nbp; b < (part + 1) * nbp; ++b) {
-                    int S = 0;
-                    unsigned c = 0;
-                    for (int j = 0; j < M; ++j) {
-                        S += (int)H[hidx(r, b * M + j, 0, lane)];
-                        c += H[hidx(r, b * M + j, 1, lane)];
+        // reduction.  Bin b = rows b*M .. b*M + M-1; a warp takes octets of bins (one
+        // 32-byte sector per output array) for all R period slots.
+        const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
+        const int octs = nb >> 3;
+        {
+            // sweep 1: sums and counts out; bin mean m (of the centred flux) back into the
+            // bin's first row as an fp64 {lo, hi} (NaN = empty); one-pass moments about the
+            // curve mean (exactly zero for a flat profile)
+            double s1[LP_R], s2[LP_R];
+            int kk[LP_R];
+#pragma unroll
+            for (int r = 0; r < LP_R; ++r) {
+                s1[r] = 0.0;
+                s2[r] = 0.0;
+                kk[r] = 0;
+            }
+            for (int oct = warp; oct < octs; oct += LP_WARPS) {
+#pragma unroll
+                for (int r = 0; r < LP_R; ++r) {
+                    const long long j = p0 + r * 32 + lane;
+                    const bool live = j < a.nperiods;
+                    const bool ok = live && valid[r];
+                    float fs[8];
+                    unsigned fc[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int row0 = (oct * 8 + e) * M;
+                        int S = 0;
+                        unsigned c = 0;
+                        for (int jj = 0; jj < M; ++jj) {
+                            const int i0 = hidx(r, row0 + jj, 0, lane);
+                            S += (int)H[i0];
+                            c += H[i0 + 32];
+                            if (jj > 0) {
+                                H[i0] = 0u;
+                                H[i0 + 32] = 0u;
+                            }
+                        }
+                        if (!ok) {
+                            S = 0;
+                            c = 0;
+                        }
+                        const double sq = __dmul_rn((double)S, inv_scale);
+                        fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
+                        fc[e] = c;
+                        const int i0 = hidx(r, row0, 0, lane);
+                        if (want_norm) {
+                            double m = CUDART_NAN;
+                            if (c > 0) {
+                                m = __ddiv_rn(sq, (double)c);
+                                const double d = __dsub_rn(m, pivot);
+                                s1[r] += d;
+                                s2[r] += __dmul_rn(d, d);
+                                kk[r] += 1;
+                            }
+                            H[i0] = (unsigned)__double2loint(m);
+                            H[i0 + 32] = (unsigned)__double2hiint(m);
+                        } else {
+                            H[i0] = 0u;
+                            H[i0 + 32] = 0u;
+                        }
                     }
-                    if (c > 0) {
-                        s1 += __ddiv_rn(__dmul_rn((double)S, inv_scale), (double)c);
-                        kk += 1;
+                    if (live) {
+                        const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
+                        if (a.out_sum) {
+                            float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
+                            o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
+                            o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
+                        }
+                        if (a.out_count) {
+                            uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
+                            o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
+                            o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
+                        }
                     }
                 }
-                part_s[part * LP_GROUP + r * 32 + lane] = s1;
-                part_k[part * LP_GROUP + r * 32 + lane] = kk;
             }
+            if (want_norm) {
+#pragma unroll
+                for (int r = 0; r < LP_R; ++r) {
+                    ps1[warp * LP_GROUP + r * 32 + lane] = s1[r];
+                    ps2[warp * LP_GROUP + r * 32 + lane] = s2[r];
+                    pkk[warp * LP_GROUP + r * 32 + lane] = kk[r];
+                }
+            }
+        }
+        if (want_norm) {
             __syncthreads();
             if (warp < LP_R) {
-                double s1 = 0.0;
+                double s1 = 0.0, s2 = 0.0;
                 int kk = 0;
-                for (int p = 0; p < LP_PARTS; ++p) {
-                    s1 += part_s[p * LP_GROUP + warp * 32 + lane];
-                    kk += part_k[p * LP_GROUP + warp * 32 + lane];
+                for (int w = 0; w < LP_WARPS; ++w) {       // fixed order: deterministic
+                    s1 += ps1[w * LP_GROUP + warp * 32 + lane];
+                    s2 += ps2[w * LP_GROUP + warp * 32 + lane];
+                    kk += pkk[w * LP_GROUP + warp * 32 + lane];
                 }
-                st_mu[warp * 32 + lane] = (kk > 0) ? __ddiv_rn(s1, (double)kk) : 0.0;
+                double mu = 0.0, isd = 0.0;
+                if (kk > 0) {
+                    const double dm = __ddiv_rn(s1, (double)kk);
+                    mu = __dadd_rn(pivot, dm);
+                    const double var = __dsub_rn(__ddiv_rn(s2, (double)kk), __dmul_rn(dm, dm));
+                    const double sd = (var > 0.0) ? sqrt(var) : 0.0;
+                    if (kk >= 2 && sd > 0.0) isd = __ddiv_rn(1.0, sd);
+                }
+                st_mu[warp * 32 + lane] = mu;
+                st_isd[warp * 32 + lane] = isd;
                 st_kk[warp * 32 + lane] = kk;
             }
             __syncthreads();
-            // sweep 2: sum of squared deviations
-            if (warp < LP_R * LP_PARTS) {
-                const double mu = st_mu[r * 32 + lane];
-                double s2 = 0.0;
-                for (int b = part * nbp; b < (part + 1) * nbp; ++b) {
-                    int S = 0;
-                    unsigned c = 0;
-                    for (int j = 0; j < M; ++j) {
-                        S += (int)H[hidx(r, b * M + j, 0, lane)];
-                        c += H[hidx(r, b * M + j, 1, lane)];
-                    }
-                    if (c > 0) {
-                        double d = __dsub_rn(__ddiv_rn(__dmul_rn((double)S, inv_scale), (double)c), mu);
-                        s2 += __dmul_rn(d, d);
-                    }
-                }
-                part_s[part * LP_GROUP + r * 32 + lane] = s2;
-            }
-            __syncthreads();
-            if (warp < LP_R) {
-                double s2 = 0.0;
-                for (int p = 0; p < LP_PARTS; ++p) s2 += part_s[p * LP_GROUP + warp * 32 + lane];
-                const int kk = st_kk[warp * 32 + lane];
-                const double sd = (kk > 0) ? sqrt(__ddiv_rn(s2, (double)kk)) : 0.0;
-                const bool flat = (kk < 2) || !(sd > 0.0);
-                st_isd[warp * 32 + lane] = flat ? 0.0 : __ddiv_rn(1.0, sd);
-            }
-            __syncthreads();
-        }
-        // sweep 3: convert, write 8 bins (one 32-byte sector per array) at a time, clear rows
-        {
-            const int octs = nb >> 3;
-            for (int unit = warp; unit < LP_R * octs; unit += LP_WARPS) {
-                const int r = unit / octs, oct = unit - r * octs;
-                const long long j = p0 + r * 32 + lane;
-                const bool live = j < a.nperiods;
-                bool ok = false;
-                if (live) {
-                    const double x = a.rp[j];
-                    ok = (x == x);
-                }
-                const double mu = a.out_norm ? st_mu[r * 32 + lane] : 0.0;
-                const double isd = a.out_norm ? st_isd[r * 32 + lane] : 0.0;
-                const int kk = a.out_norm ? st_kk[r * 32 + lane] : 0;
-                float fs[8], fn[8];
-                unsigned fc[8];
+            // sweep 2: normalised profile out, rows cleared
+            for (int oct = warp; oct < octs; oct += LP_WARPS) {
 #pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int b = oct * 8 + e;
-                    int S = 0;
-                    unsigned c = 0;
-                    for (int jj = 0; jj < M; ++jj) {
-                        const int i0 = hidx(r, b * M + jj, 0, lane);
-                        S += (int)H[i0];
-                        c += H[i0 + 32];
+                for (int r = 0; r < LP_R; ++r) {
+                    const long long j = p0 + r * 32 + lane;
+                    const bool live = j < a.nperiods;
+                    const double mu = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
+                    const double base_o = (live && valid[r] && st_kk[r * 32 + lane] > 0)
+                                              ? __dadd_rn(mu, center) : 0.0;
+                    float fn[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int i0 = hidx(r, (oct * 8 + e) * M, 0, lane);
+                        const double m = __hiloint2double((int)H[i0 + 32], (int)H[i0]);
                         H[i0] = 0u;
                         H[i0 + 32] = 0u;
+                        double o = base_o;
+                        if (m == m && isd > 0.0) o = __dadd_rn(o, __dmul_rn(__dsub_rn(m, mu), isd));
+                        fn[e] = (float)o;
                     }
-                    if (!ok) {
-                        S = 0;
-                        c = 0;
-                    }
-                    const double sq = __dmul_rn((double)S, inv_scale);
-                    fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
-                    fc[e] = c;
-                    double o = 0.0;
-                    if (ok && kk > 0) {
-                        o = __dadd_rn(mu, center);
-                        if (c > 0 && isd > 0.0)
-                            o = __dadd_rn(o, __dmul_rn(__dsub_rn(__ddiv_rn(sq, (double)c), mu), isd));
-                    }
-                    fn[e] = (float)o;
-                }
-                if (live) {
-                    const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
-                    if (a.out_sum) {
-                        float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
-                        o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
-                        o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
-                    }
-                    if (a.out_count) {
-                        uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
-                        o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
-                        o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
-                    }
-                    if (a.out_norm) {
-                        float4 *o4 = reinterpret_cast<float4 *>(a.out_norm + off);
+                    if (live) {
+                        float4 *o4 = reinterpret_cast<float4 *>(
+                            a.out_norm + ((curve * a.nperiods + j) * nb) + oct * 8);
                         o4[0] = make_float4(fn[0], fn[1], fn[2], fn[3]);
                         o4[1] = make_float4(fn[4], fn[5], fn[6], fn[7]);
                     }

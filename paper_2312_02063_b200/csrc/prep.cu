@@ -123,6 +123,7 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
     // pass 3: ordered compaction + conversion
     if (tid == 0) tile_base = 0;
     __syncthreads();
+    double qsum = 0.0;
     for (long long b = 0; b < n; b += PREP_THREADS) {
         long long i = b + tid;
         bool ok = false;
@@ -148,6 +149,7 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
             long long o = start + base + wbase + wpos;
             s.u[o] = u;
             s.q[o] = q;
+            qsum += (double)q;
         }
         __syncthreads();
         if (tid == PREP_THREADS - 1) tile_base = base + wbase + __popc(bal);
@@ -157,6 +159,8 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
     // record {v = u - a, q}.  (The compacted u / q were written by this CTA above.)
     const int n_valid = tile_base;
     const long long tile0 = start / GPFC_TILE + c;   // disjoint per curve: ceil(n/T) <= n/T + 1
+    const long long rec0 = (start + c + 1) & ~1LL;   // even, disjoint per curve
+    qsum = block_sum(qsum, red);                     // exact: |sum q| < 2^31
     double span_max = 0.0;
     for (int t = warp; t * GPFC_TILE < n_valid; t += PREP_THREADS / 32) {
         const int base = t * GPFC_TILE;
@@ -176,21 +180,29 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
             lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
             hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
         }
+        const double span = __dsub_ru(hi, lo);
+        int e = 0;
+        (void)frexp(span, &e);                 // span < 2^e
+        int S = 32 - e;                        // span * 2^S < 2^32
+        if (S > 40) S = 40;
+        if (S < -900) S = -900;
+        const double scale = ldexp(1.0, S);
 #pragma unroll
         for (int k = 0; k < GPFC_TILE / 32; ++k) {
             int i = base + k * 32 + lane;
             if (i < n_valid) {
-                double v = __dsub_rn(uu[k], lo);
-                s.rec[start + i] = make_int4(__double2loint(v), __double2hiint(v), s.q[start + i], 0);
+                double w = rint(__dmul_rn(__dsub_rn(uu[k], lo), scale));
+                if (w > 4294967295.0) w = 4294967295.0;
+                s.rec[rec0 + i] = make_int2((int)(unsigned)w, s.q[start + i]);
             }
         }
         if (lane == 0) {
             TileInfo ti;
             ti.a = lo;
-            ti.span = __dsub_ru(hi, lo);
+            ti.inv_scale = ldexp(1.0, -S);
             s.tiles[tile0 + t] = ti;
         }
-        span_max = fmax(span_max, __dsub_ru(hi, lo));
+        span_max = fmax(span_max, span);
     }
     if (lane == 0) warp_span[warp] = span_max;
     __syncthreads();
@@ -198,6 +210,8 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
         for (int w = 0; w < PREP_THREADS / 32; ++w) span_max = fmax(span_max, warp_span[w]);
         CurveMeta m;
         m.start = start;
+        m.rec0 = rec0;
+        m.pivot = (tile_base > 0) ? __ddiv_rn(__dmul_rn(qsum, ldexp(1.0, -shift)), (double)tile_base) : 0.0;
         m.tile0 = tile0;
         m.span_max = span_max;
         m.n_valid = tile_base;
