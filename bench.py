@@ -71,6 +71,18 @@ def make_workload(args, rank):
     return workloads.make(args.config, **kw)
 
 
+def max_over_ranks(value, world, device=None):
+    """Max of a per-rank scalar over all ranks (no-op for world == 1).  The tensor lives on
+    `device` (cuda under NCCL, cpu under gloo)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
 def workload_desc(w, args):
     d = {"workload": "BASELINE.json configs[%d] %s" % (w.config_id, w.name),
          "curves": w.ncurves, "samples_per_curve": int(w.n_total // max(w.ncurves, 1)),
@@ -140,35 +152,37 @@ class ClockSampler:
 
 # --------------------------------------------------------------------------- oracle legs
 def oracle_sample(w, periods_host, budget_pp):
-    """Bounded sample of the workload for the CPU oracle: the first curve(s) and the
-    first periods, about `budget_pp` point-periods."""
+    """Bounded sample of the workload for the CPU oracle: the first curves and the first
+    periods, about `budget_pp` point-periods -> (ncurves, nperiods)."""
     n0 = int(w.offsets[1] - w.offsets[0]) if w.ncurves else 0
     npd = int(min(w.nperiods, max(1, budget_pp // max(n0, 1))))
-    return 1 if w.ncurves else 0, npd
+    nc = int(min(w.ncurves, max(1, budget_pp // max(n0 * npd, 1))))
+    return nc, npd
 
 
 def run_oracle(w, periods_host, ncurves, npd, threads):
-    """Oracle fold + normalise of `ncurves` curves x first `npd` periods, the period axis
-    split over a thread pool (each chunk is the plain single-threaded C routine)."""
+    """Oracle fold + normalise of the first `ncurves` curves x first `npd` periods.  Tasks
+    (one curve x one slice of the period axis) go to a thread pool; each task is the plain
+    single-threaded C routine (ctypes releases the GIL)."""
     from concurrent.futures import ThreadPoolExecutor
     from oracle import ref
-    off = w.offsets[:ncurves + 1]
-    t = w.times[:off[-1]]
-    f = w.flux[:off[-1]]
     per = np.ascontiguousarray(periods_host[:npd])
-    nchunks = max(1, min(npd, threads))
-    edges = np.linspace(0, npd, nchunks + 1).astype(np.int64)
+    nsl = max(1, min(npd, -(-threads // max(ncurves, 1))))
+    edges = np.linspace(0, npd, nsl + 1).astype(np.int64)
+    tasks = [(c, int(edges[i]), int(edges[i + 1])) for c in range(ncurves) for i in range(nsl)]
 
-    def work(i):
-        lo, hi = int(edges[i]), int(edges[i + 1])
+    def work(task):
+        c, lo, hi = task
         if hi > lo:
-            ref.fold_batch(t, f, off, per[lo:hi], w.nbins, want_norm=True, want64=False)
+            a, b = int(w.offsets[c]), int(w.offsets[c + 1])
+            ref.fold_batch(w.times[a:b], w.flux[a:b], np.array([0, b - a], np.int64), per[lo:hi],
+                           w.nbins, want_norm=True, want64=False)
 
     t0 = time.perf_counter()
     with ThreadPoolExecutor(max_workers=threads) as ex:
-        list(ex.map(work, range(nchunks)))
+        list(ex.map(work, tasks))
     dt = time.perf_counter() - t0
-    pp = int(off[-1]) * npd
+    pp = int(w.offsets[ncurves]) * npd
     return pp, dt
 
 
@@ -183,8 +197,8 @@ def cpu_baseline(w, periods_host):
     nc, npd = oracle_sample(w, periods_host, int(rate0 * 15.0))
     pp, dt = run_oracle(w, periods_host, nc, npd, cores)
     return {"value": pp / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": "curve 0 x first %d periods (%.3g point-periods, %.1f s), fold + normalise, "
-                      "period axis split over %d threads" % (npd, pp, dt, cores)}
+            "sample": "first %d curve(s) x first %d periods (%.3g point-periods, %.1f s), fold + "
+                      "normalise, %d threads" % (nc, npd, pp, dt, cores)}
 
 
 def reference_arm(args):
@@ -209,8 +223,8 @@ def reference_arm(args):
         pps += pp
         dts += dt
     value = pps / max(dts, 1e-12)
-    sample = ("each step: curve 0 x first %d periods (%.3g point-periods), fold + normalise, "
-              "%d threads" % (npd, float(pp), cores))
+    sample = ("each step: first %d curve(s) x first %d periods (%.3g point-periods), fold + "
+              "normalise, %d threads" % (nc, npd, float(pp), cores))
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": 1e3 * dts / max(args.steps, 1), "higher_is_better": True,
@@ -287,10 +301,7 @@ def gpu_arm(args):
     prof = gp.gpfc_profile_read()
     gp.gpfc_profile(False)
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        tt = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
+    ms = max_over_ranks(ms, world, "cuda")
     pp_step_all = float(w.point_periods) * world
     value = pp_step_all * args.steps / (ms * 1e-3)
 
@@ -301,11 +312,11 @@ def gpu_arm(args):
         torch.cuda.empty_cache()
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
         h_t, h_f, h_o = pin(w.times), pin(w.flux), pin(w.offsets)
-        h_norm = torch.empty(shape, dtype=torch.float32).pin_memory()
+        h_norm = torch.empty(shape, dtype=torch.float32, pin_memory=True)
         h_sum = h_cnt = None
         if not w.fused_normalize:
-            h_sum = torch.empty(shape, dtype=torch.float32).pin_memory()
-            h_cnt = torch.empty(shape, dtype=torch.int32).pin_memory()
+            h_sum = torch.empty(shape, dtype=torch.float32, pin_memory=True)
+            h_cnt = torch.empty(shape, dtype=torch.int32, pin_memory=True)
 
         def step_host():
             per = gp.gpfc_make_period_grid_host(w.pmin, w.pmax, w.nperiods, w.grid_mode)
@@ -322,10 +333,7 @@ def gpu_arm(args):
             step_host()
         barrier()
         dt = time.perf_counter() - t0
-        if world > 1:
-            tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt = float(tt.item())
+        dt = max_over_ranks(dt, world, "cuda")
         nout = int(np.prod(shape)) * 4
         e2e = {"value": pp_step_all * nstep / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(w.n_total * 12 + w.offsets.nbytes),
@@ -347,7 +355,7 @@ def gpu_arm(args):
     roof = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_nominal / 1e9,
             "unit": "G shared-atomic lane-updates/s", "frac": achieved / peak_nominal,
             "traffic": None,
-            "kernel": "fold_cols_kernel", "kernel_ms": fold_ms,
+            "kernel": "fold_lp_kernel" if w.nbins in (32, 64, 128, 256) else "fold_cols_kernel", "kernel_ms": fold_ms,
             "peak_source": "derived: 148 SMs x 32 lanes/clk x %.0f MHz" % sm_max,
             "hbm_bound": {"algorithmic_bytes": out_bytes + w.n_total * 12.0,
                           "achieved_gbs": (out_bytes + w.n_total * 12.0) / (fold_ms * 1e-3) / 1e9}}

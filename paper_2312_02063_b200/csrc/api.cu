@@ -257,6 +257,9 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
                          int64_t nperiods, int nbins, const double *t0, float *out_sum,
                          uint32_t *out_count, float *out_norm)
 {
+    // Streaming host path: inputs go up once; the curves are folded in chunks whose outputs
+    // land in one of two device slabs, and the device->host copy of chunk k (copy stream)
+    // overlaps the fold of chunk k+1 (the caller's stream).
     if (ncurves < 0 || nperiods < 0 || n_total < 0)
         return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
     if (nbins < 1 || nbins > GPFC_MAX_NBINS)
@@ -264,14 +267,21 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
     if (ncurves == 0 || nperiods == 0) return GPFC_OK;
     if (!offsets || !periods || (n_total > 0 && (!times || !flux)))
         return fail(GPFC_ERR_INVALID_ARG, "NULL pointer%s");
+    for (int64_t c = 0; c < ncurves; ++c)
+        if (offsets[c + 1] < offsets[c] || offsets[c] < 0 || offsets[c + 1] > n_total)
+            return fail(GPFC_ERR_INVALID_ARG, "offsets must be non-decreasing within [0, n_total]%s");
     cudaStream_t st = g_ts.stream;
-    const size_t nout = (size_t)ncurves * (size_t)nperiods * (size_t)nbins;
+    const int nout = (out_sum ? 1 : 0) + (out_count ? 1 : 0) + (out_norm ? 1 : 0);
+    const size_t row = (size_t)nperiods * (size_t)nbins;      // elements per curve and array
+    // chunk: about 512 MB of output per slab, at least one curve
+    int64_t chunk = nout ? (int64_t)((size_t)(512u << 20) / (row * 4 * (size_t)nout)) : ncurves;
+    if (chunk < 1) chunk = 1;
+    if (chunk > ncurves) chunk = ncurves;
     const size_t b_t = align_up((size_t)n_total * 8), b_f = align_up((size_t)n_total * 4);
     const size_t b_o = align_up((size_t)(ncurves + 1) * 8), b_p = align_up((size_t)nperiods * 8);
     const size_t b_t0 = t0 ? align_up((size_t)ncurves * 8) : 0;
-    const size_t b_out = align_up(nout * 4);
-    size_t total = b_t + b_f + b_o + b_p + b_t0 + 256;
-    total += (out_sum ? b_out : 0) + (out_count ? b_out : 0) + (out_norm ? b_out : 0);
+    const size_t b_arr = align_up((size_t)chunk * row * 4);
+    const size_t total = b_t + b_f + b_o + b_p + b_t0 + 2 * (size_t)nout * b_arr + 256;
     char *base = nullptr;
     cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&base), total, st);
     if (e != cudaSuccess) {
@@ -285,14 +295,22 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
     double *d_p = reinterpret_cast<double *>(cur); cur += b_p;
     double *d_t0 = nullptr;
     if (t0) { d_t0 = reinterpret_cast<double *>(cur); cur += b_t0; }
-    float *d_sum = nullptr, *d_norm = nullptr;
-    uint32_t *d_cnt = nullptr;
-    if (out_sum) { d_sum = reinterpret_cast<float *>(cur); cur += b_out; }
-    if (out_count) { d_cnt = reinterpret_cast<uint32_t *>(cur); cur += b_out; }
-    if (out_norm) { d_norm = reinterpret_cast<float *>(cur); cur += b_out; }
+    char *slab[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
+    for (int s = 0; s < 2; ++s)
+        for (int k = 0; k < 3; ++k) {
+            const bool want = (k == 0 && out_sum) || (k == 1 && out_count) || (k == 2 && out_norm);
+            if (want) { slab[s][k] = cur; cur += b_arr; }
+        }
 
+    cudaStream_t cs = nullptr;
+    cudaEvent_t done[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr};
+    e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+    for (int s = 0; s < 2 && e == cudaSuccess; ++s) {
+        e = cudaEventCreateWithFlags(&done[s], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&freed[s], cudaEventDisableTiming);
+    }
     int rc = GPFC_OK;
-    if (n_total > 0) {
+    if (e == cudaSuccess && n_total > 0) {
         e = cudaMemcpyAsync(d_t, times, (size_t)n_total * 8, cudaMemcpyHostToDevice, st);
         if (e == cudaSuccess)
             e = cudaMemcpyAsync(d_f, flux, (size_t)n_total * 4, cudaMemcpyHostToDevice, st);
@@ -303,21 +321,42 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
         e = cudaMemcpyAsync(d_p, periods, (size_t)nperiods * 8, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess && t0)
         e = cudaMemcpyAsync(d_t0, t0, (size_t)ncurves * 8, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) {
-        rc = fold_device(d_t, d_f, d_o, ncurves, n_total, d_p, nperiods, nbins, d_t0, 0.0, d_sum,
-                         d_cnt, d_norm);
-        if (rc == GPFC_OK) {
-            if (out_sum) e = cudaMemcpyAsync(out_sum, d_sum, nout * 4, cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess && out_count)
-                e = cudaMemcpyAsync(out_count, d_cnt, nout * 4, cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess && out_norm)
-                e = cudaMemcpyAsync(out_norm, d_norm, nout * 4, cudaMemcpyDeviceToHost, st);
-        }
+    int64_t k = 0;
+    for (int64_t c0 = 0; c0 < ncurves && e == cudaSuccess && rc == GPFC_OK; c0 += chunk, ++k) {
+        const int s = (int)(k & 1);
+        const int64_t nc = (ncurves - c0 < chunk) ? ncurves - c0 : chunk;
+        if (k >= 2) e = cudaStreamWaitEvent(st, freed[s], 0);     // slab s copied out
+        if (e != cudaSuccess) break;
+        // the prepass scratch covers the samples offsets[c0] .. offsets[c0 + nc]: pass the
+        // whole arrays (offsets are absolute) and size the scratch by n_total
+        rc = fold_device(d_t, d_f, d_o + c0, nc, n_total, d_p, nperiods, nbins,
+                         d_t0 ? d_t0 + c0 : nullptr, 0.0,
+                         reinterpret_cast<float *>(slab[s][0]),
+                         reinterpret_cast<uint32_t *>(slab[s][1]),
+                         reinterpret_cast<float *>(slab[s][2]));
+        if (rc != GPFC_OK) break;
+        e = cudaEventRecord(done[s], st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, done[s], 0);
+        const size_t bytes = (size_t)nc * row * 4, off = (size_t)c0 * row;
+        if (e == cudaSuccess && out_sum)
+            e = cudaMemcpyAsync(out_sum + off, slab[s][0], bytes, cudaMemcpyDeviceToHost, cs);
+        if (e == cudaSuccess && out_count)
+            e = cudaMemcpyAsync(out_count + off, slab[s][1], bytes, cudaMemcpyDeviceToHost, cs);
+        if (e == cudaSuccess && out_norm)
+            e = cudaMemcpyAsync(out_norm + off, slab[s][2], bytes, cudaMemcpyDeviceToHost, cs);
+        if (e == cudaSuccess) e = cudaEventRecord(freed[s], cs);
     }
+    cudaError_t e2 = cs ? cudaStreamSynchronize(cs) : cudaSuccess;
+    cudaError_t e3 = cudaStreamSynchronize(st);
     cudaFreeAsync(base, st);
-    cudaError_t e2 = cudaStreamSynchronize(st);
+    for (int s = 0; s < 2; ++s) {
+        if (done[s]) cudaEventDestroy(done[s]);
+        if (freed[s]) cudaEventDestroy(freed[s]);
+    }
+    if (cs) cudaStreamDestroy(cs);
     if (rc != GPFC_OK) return rc;
     if (e == cudaSuccess) e = e2;
+    if (e == cudaSuccess) e = e3;
     if (e != cudaSuccess) return cuda_fail(e, "host-buffer fold");
     return GPFC_OK;
 }
