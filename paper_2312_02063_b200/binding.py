@@ -106,6 +106,17 @@ def gpfc_version() -> str:
     return lib().gpfc_version().decode()
 
 
+def gpfc_last_error() -> str:
+    return lib().gpfc_last_error().decode("utf-8", "replace")
+
+
+def gpfc_set_stream(stream=None) -> None:
+    """stream: a torch.cuda.Stream (None = torch's current stream).  The other wrappers call
+    this with the current stream before every launch."""
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(lib().gpfc_set_stream(ctypes.c_void_p(st.cuda_stream)), "gpfc_set_stream")
+
+
 def gpfc_n_sample(n_o: float, t_window: float, l_width: float) -> float:
     return float(lib().gpfc_n_sample(n_o, t_window, l_width))
 
