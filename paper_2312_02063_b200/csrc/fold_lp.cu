@@ -34,8 +34,9 @@ namespace gpfc {
 
 namespace {
 
-constexpr int LP_THREADS = 512;
+constexpr int LP_THREADS = 768;
 constexpr int LP_WARPS = LP_THREADS / 32;
+constexpr int LP_EPI_WARPS = 16;             // warps that run the epilogue sweeps
 constexpr int LP_R = 3;                       // periods per lane
 constexpr int LP_GROUP = 32 * LP_R;           // periods per work item
 constexpr int LP_ROWS = 256;                  // rows per period (fold resolution)
@@ -46,10 +47,10 @@ constexpr int LP_HIST_BYTES = LP_R * LP_ROWS * 256;           // 196,608
 // scratch after the histograms: sample staging during the fold, statistics partials in the
 // epilogue (the two never live at the same time)
 constexpr int LP_STAGE_OFF = LP_HIST_BYTES;                   // int2 [LP_WARPS][LP_GRAN]
-constexpr int LP_PS1_OFF = LP_HIST_BYTES;                     // double [LP_WARPS][LP_GROUP]
-constexpr int LP_PS2_OFF = LP_PS1_OFF + LP_WARPS * LP_GROUP * 8;
-constexpr int LP_PKK_OFF = LP_PS2_OFF + LP_WARPS * LP_GROUP * 8;      // int [LP_WARPS][LP_GROUP]
-constexpr int LP_MU_OFF = LP_PKK_OFF + LP_WARPS * LP_GROUP * 4;       // double [LP_GROUP]
+constexpr int LP_PS1_OFF = LP_HIST_BYTES;                     // double [LP_EPI_WARPS][LP_GROUP]
+constexpr int LP_PS2_OFF = LP_PS1_OFF + LP_EPI_WARPS * LP_GROUP * 8;
+constexpr int LP_PKK_OFF = LP_PS2_OFF + LP_EPI_WARPS * LP_GROUP * 8;  // int [LP_EPI_WARPS][LP_GROUP]
+constexpr int LP_MU_OFF = LP_PKK_OFF + LP_EPI_WARPS * LP_GROUP * 4;       // double [LP_GROUP]
 constexpr int LP_ISD_OFF = LP_MU_OFF + LP_GROUP * 8;                  // double [LP_GROUP]
 constexpr int LP_KK_OFF = LP_ISD_OFF + LP_GROUP * 8;                  // int [LP_GROUP]
 constexpr int LP_CTR_OFF = LP_KK_OFF + LP_GROUP * 4;
@@ -302,7 +303,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 s2[r] = 0.0;
                 kk[r] = 0;
             }
-            for (int oct = warp; oct < octs; oct += LP_WARPS) {
+            for (int oct = warp; oct < octs && warp < LP_EPI_WARPS; oct += LP_EPI_WARPS) {
 #pragma unroll
                 for (int r = 0; r < LP_R; ++r) {
                     const long long j = p0 + r * 32 + lane;
@@ -363,7 +364,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     }
                 }
             }
-            if (want_norm) {
+            if (want_norm && warp < LP_EPI_WARPS) {
 #pragma unroll
                 for (int r = 0; r < LP_R; ++r) {
                     ps1[warp * LP_GROUP + r * 32 + lane] = s1[r];
@@ -377,7 +378,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
             if (warp < LP_R) {
                 double s1 = 0.0, s2 = 0.0;
                 int kk = 0;
-                for (int w = 0; w < LP_WARPS; ++w) {       // fixed order: deterministic
+                for (int w = 0; w < LP_EPI_WARPS; ++w) {   // fixed order: deterministic
                     s1 += ps1[w * LP_GROUP + warp * 32 + lane];
                     s2 += ps2[w * LP_GROUP + warp * 32 + lane];
                     kk += pkk[w * LP_GROUP + warp * 32 + lane];
@@ -396,7 +397,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
             }
             __syncthreads();
             // sweep 2: normalised profile out, rows cleared
-            for (int oct = warp; oct < octs; oct += LP_WARPS) {
+            for (int oct = warp; oct < octs && warp < LP_EPI_WARPS; oct += LP_EPI_WARPS) {
 #pragma unroll
                 for (int r = 0; r < LP_R; ++r) {
                     const long long j = p0 + r * 32 + lane;
