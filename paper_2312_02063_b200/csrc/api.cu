@@ -126,6 +126,8 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
         a.out_sum = out_sum;
         a.out_count = out_count;
         a.out_norm = out_norm;
+        a.n_min = 0;
+        a.n_max = 0x7fffffff;
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (g_ts.profiling && cudaEventCreate(&e0) == cudaSuccess &&
             cudaEventCreate(&e1) == cudaSuccess)

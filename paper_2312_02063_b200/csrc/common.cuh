@@ -60,6 +60,7 @@ struct FoldArgs {
     float *out_sum;
     uint32_t *out_count;
     float *out_norm;
+    int n_min, n_max;   // a launch handles the curves with n_min <= n_valid <= n_max
 };
 
 // ---- exact bin of one sample: the formula of include/gpfc.h, every operation
@@ -164,7 +165,9 @@ cudaError_t launch_prep(const double *times, const float *flux, const int64_t *o
                         cudaStream_t st);
 cudaError_t launch_fold(const FoldArgs &a, cudaStream_t st);
 cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st);   // fold_lp.cu: nbins in {32,64,128,256}
+cudaError_t launch_fold_generic(const FoldArgs &a, cudaStream_t st);   // fold.cu: any nbins, exact formula
 bool fold_lp_handles(int nbins);
+int fold_lp_rows(int nbins);   // fold resolution of the lane-period kernel (256 or 1024)
 int num_sms();
 cudaError_t launch_normalize(const float *sum, const uint32_t *count, long long nprofiles,
                              int nbins, float *out, cudaStream_t st);

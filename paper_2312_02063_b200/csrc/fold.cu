@@ -254,6 +254,7 @@ fold_generic_kernel(FoldArgs a, long long nitems)
         const long long curve = item / a.nperiods;
         const long long j = item - curve * a.nperiods;
         const CurveMeta m = a.meta[curve];
+        if (m.n_valid < a.n_min || m.n_valid > a.n_max) continue;   // another launch owns it
         const double per = a.periods[j];
         if (period_ok(per)) {
             const double *__restrict__ u = a.u + m.start;
@@ -317,12 +318,16 @@ cudaError_t launch_fold(const FoldArgs &a, cudaStream_t st)
     if (a.ncurves <= 0 || a.nperiods <= 0) return cudaSuccess;
     if (fold_lp_handles(a.nbins)) return launch_fold_lp(a, st);
     switch (a.nbins) {
-        case 512: return launch_cols<9, 5, 1, 4>(a, st);
-        case 1024: return launch_cols<10, 4, 1, 4>(a, st);
         case 2048: return launch_cols<11, 3, 1, 4>(a, st);
         case 4096: return launch_cols<12, 2, 1, 4>(a, st);
         default: break;
     }
+    return launch_fold_generic(a, st);
+}
+
+cudaError_t launch_fold_generic(const FoldArgs &a, cudaStream_t st)
+{
+    if (a.ncurves <= 0 || a.nperiods <= 0) return cudaSuccess;
     long long nitems = a.ncurves * a.nperiods;
     long long cap = (long long)num_sms() * 8;
     long long grid = nitems < cap ? nitems : cap;

@@ -36,24 +36,40 @@ namespace {
 
 constexpr int LP_THREADS = 768;
 constexpr int LP_WARPS = LP_THREADS / 32;
-constexpr int LP_EPI_WARPS = 16;             // warps that run the epilogue sweeps
-constexpr int LP_R = 3;                       // periods per lane
-constexpr int LP_GROUP = 32 * LP_R;           // periods per work item
-constexpr int LP_ROWS = 256;                  // rows per period (fold resolution)
+constexpr int LP_EPI_WARPS = 16;              // warps that run the epilogue sweeps
 constexpr int LP_GRAN = 64;                   // samples per staging granule
 constexpr unsigned LP_SMEM_BASE = 0x400;      // shared-window address of dynamic shared memory
 
-constexpr int LP_HIST_BYTES = LP_R * LP_ROWS * 256;           // 196,608
+// Two variants of the kernel:
+//   VAR 0: 256 rows, R = 3 periods per lane, histogram [r][row][sum|count][lane] (nbins 32..256)
+//   VAR 1: 1024 rows, R = 1, sums [row][lane] (128 KB) and PACKED counts [row & 511][lane]
+//          (64 KB): the low half-word counts rows k and k + 512 together, the high half-word
+//          counts row k + 512, so a curve may have at most 65,535 valid samples
+//          (nbins 512, 1024; longer curves are left to fold_generic_kernel).
+template <int VAR> struct LpV;
+template <> struct LpV<0> {
+    static constexpr int R = 3, ROWLOG = 8;
+    static constexpr bool PACKED = false;
+};
+template <> struct LpV<1> {
+    static constexpr int R = 1, ROWLOG = 10;
+    static constexpr bool PACKED = true;
+};
+constexpr int LP_GROUP_MAX = 96;              // periods per work item, largest variant
+constexpr int LP_PACKED_MAX_N = 65535;
+
+constexpr int LP_HIST_BYTES = 196608;         // both variants
+constexpr int LP_CNT1_OFF = 131072;           // VAR 1: byte offset of the packed counts
 // scratch after the histograms: sample staging during the fold, statistics partials in the
 // epilogue (the two never live at the same time)
 constexpr int LP_STAGE_OFF = LP_HIST_BYTES;                   // int2 [LP_WARPS][LP_GRAN]
-constexpr int LP_PS1_OFF = LP_HIST_BYTES;                     // double [LP_EPI_WARPS][LP_GROUP]
-constexpr int LP_PS2_OFF = LP_PS1_OFF + LP_EPI_WARPS * LP_GROUP * 8;
-constexpr int LP_PKK_OFF = LP_PS2_OFF + LP_EPI_WARPS * LP_GROUP * 8;  // int [LP_EPI_WARPS][LP_GROUP]
-constexpr int LP_MU_OFF = LP_PKK_OFF + LP_EPI_WARPS * LP_GROUP * 4;       // double [LP_GROUP]
-constexpr int LP_ISD_OFF = LP_MU_OFF + LP_GROUP * 8;                  // double [LP_GROUP]
-constexpr int LP_KK_OFF = LP_ISD_OFF + LP_GROUP * 8;                  // int [LP_GROUP]
-constexpr int LP_CTR_OFF = LP_KK_OFF + LP_GROUP * 4;
+constexpr int LP_PS1_OFF = LP_HIST_BYTES;                     // double [LP_EPI_WARPS][GROUP]
+constexpr int LP_PS2_OFF = LP_PS1_OFF + LP_EPI_WARPS * LP_GROUP_MAX * 8;
+constexpr int LP_PKK_OFF = LP_PS2_OFF + LP_EPI_WARPS * LP_GROUP_MAX * 8;   // int [LP_EPI_WARPS][GROUP]
+constexpr int LP_MU_OFF = LP_PKK_OFF + LP_EPI_WARPS * LP_GROUP_MAX * 4;    // double [GROUP]
+constexpr int LP_ISD_OFF = LP_MU_OFF + LP_GROUP_MAX * 8;                   // double [GROUP]
+constexpr int LP_KK_OFF = LP_ISD_OFF + LP_GROUP_MAX * 8;                   // int [GROUP]
+constexpr int LP_CTR_OFF = LP_KK_OFF + LP_GROUP_MAX * 4;
 constexpr int LP_SMEM_BYTES = LP_CTR_OFF + 16;
 static_assert(LP_SMEM_BYTES <= 227 * 1024, "shared memory budget");
 static_assert(LP_WARPS * LP_GRAN * 8 <= LP_MU_OFF - LP_STAGE_OFF, "staging fits in the scratch");
@@ -70,45 +86,97 @@ __device__ __forceinline__ void red_inc(unsigned addr)
     asm volatile("red.shared.add.u32 [%0+%1], 1;" ::"r"(addr), "n"(IMM) : "memory");
 }
 
-// word index of (r, row, array, lane) in the histogram
+// word index of (r, row, array, lane) in the VAR 0 histogram
 __device__ __forceinline__ int hidx(int r, int row, int arr, int lane)
 {
-    return r * (LP_ROWS * 64) + row * 64 + arr * 32 + lane;
+    return r * (256 * 64) + row * 64 + arr * 32 + lane;
+}
+
+// generic (slow-path) update of one sample: move = +1 adds it to `row`, -1 removes it
+template <int VAR>
+__device__ __forceinline__ void hist_update(unsigned *H, int r, int row, int lane, int q, int move)
+{
+    if (VAR == 0) {
+        atomicAdd(&H[hidx(r, row, 0, lane)], (unsigned)(move * q));
+        atomicAdd(&H[hidx(r, row, 1, lane)], (unsigned)move);
+    } else {
+        atomicAdd(&H[row * 32 + lane], (unsigned)(move * q));
+        atomicAdd(&H[LP_CNT1_OFF / 4 + (row & 511) * 32 + lane],
+                  (unsigned)(move * (1 + ((row >> 9) << 16))));
+    }
+}
+
+// one bin = M consecutive rows: exact sum and count
+template <int VAR>
+__device__ __forceinline__ void read_bin(const unsigned *H, int r, int row0, int M, int lane, int &S,
+                                         unsigned &c)
+{
+    S = 0;
+    c = 0;
+    for (int jj = 0; jj < M; ++jj) {
+        const int row = row0 + jj;
+        if (VAR == 0) {
+            const int i0 = hidx(r, row, 0, lane);
+            S += (int)H[i0];
+            c += H[i0 + 32];
+        } else {
+            S += (int)H[row * 32 + lane];
+            const unsigned w = H[LP_CNT1_OFF / 4 + (row & 511) * 32 + lane];
+            c += (row >> 9) ? (w >> 16) : ((w & 0xffffu) - (w >> 16));
+        }
+    }
 }
 
 // one point-period of the fast path for period slot r (compile-time)
-template <int r>
+// the constant 1 in a register the compiler cannot fold, so that (t7 & 0x10000) | 1 is ONE LOP3
+__device__ __forceinline__ unsigned opaque_one()
+{
+    unsigned one;
+    asm volatile("mov.u32 %0, 1;" : "=r"(one));
+    return one;
+}
+
+template <int VAR, int r>
 __device__ __forceinline__ void pp_update(double v, int q, double rp, double C, unsigned lane4,
-                                          unsigned &gmin)
+                                          unsigned one, unsigned &gmin)
 {
     double m = __fma_rd(v, rp, C);
     unsigned lo = (unsigned)__double2loint(m), hi = (unsigned)__double2hiint(m);
-    unsigned addr = __byte_perm(lane4, hi, 0x3240);      // (row << 8) | (lane << 2)
     gmin = min(gmin, lo);
-    red_add<(int)LP_SMEM_BASE + r * 65536>(addr, q);
-    red_inc<(int)LP_SMEM_BASE + r * 65536 + 128>(addr);
+    if (VAR == 0) {
+        unsigned addr = __byte_perm(lane4, hi, 0x3240);      // (row << 8) | (lane << 2)
+        red_add<(int)LP_SMEM_BASE + r * 65536>(addr, q);
+        red_inc<(int)LP_SMEM_BASE + r * 65536 + 128>(addr);
+    } else {
+        const unsigned t7 = hi << 7;                         // row << 7 (+ junk above bit 16)
+        const unsigned saddr = (t7 & 0x1ff80u) | lane4;      // row * 128 + lane * 4
+        const unsigned caddr = (t7 & 0x0ff80u) | lane4;      // (row & 511) * 128 + lane * 4
+        const unsigned val = (t7 & 0x10000u) | one;          // 1 + ((row >> 9) << 16)
+        red_add<(int)LP_SMEM_BASE>(saddr, q);
+        red_add<(int)LP_SMEM_BASE + LP_CNT1_OFF>(caddr, (int)val);
+    }
 }
 
-template <int r0>
+template <int VAR, int r0>
 struct ForR {
-    __device__ __forceinline__ static void run(double v, int q, const double (&rp)[LP_R],
-                                               const double (&C)[LP_R], unsigned lane4,
-                                               unsigned (&gmin)[LP_R])
+    static constexpr int R = LpV<VAR>::R;
+    __device__ __forceinline__ static void run(double v, int q, const double (&rp)[R],
+                                               const double (&C)[R], unsigned lane4,
+                                               unsigned one, unsigned (&gmin)[R])
     {
-        pp_update<r0>(v, q, rp[r0], C[r0], lane4, gmin[r0]);
-        ForR<r0 + 1>::run(v, q, rp, C, lane4, gmin);
+        if constexpr (r0 < R) {
+            pp_update<VAR, r0>(v, q, rp[r0], C[r0], lane4, one, gmin[r0]);
+            ForR<VAR, r0 + 1>::run(v, q, rp, C, lane4, one, gmin);
+        }
     }
 };
-template <>
-struct ForR<LP_R> {
-    __device__ __forceinline__ static void run(double, int, const double (&)[LP_R],
-                                               const double (&)[LP_R], unsigned,
-                                               unsigned (&)[LP_R]) {}
-};
 
+template <int VAR>
 __global__ void __launch_bounds__(LP_THREADS, 1)
 fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
 {
+    using V = LpV<VAR>;
+    constexpr int LP_R = V::R, LP_ROWS = 1 << V::ROWLOG, LP_GROUP = 32 * V::R;
     extern __shared__ __align__(1024) unsigned char smem[];
     if (probe) {   // report where dynamic shared memory starts (host checks LP_SMEM_BASE once)
         if (threadIdx.x == 0 && blockIdx.x == 0) *probe = (unsigned)__cvta_generic_to_shared(smem);
@@ -125,15 +193,17 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned lane4 = (unsigned)lane << 2;
+    const unsigned one = opaque_one();
     int4 *stage = reinterpret_cast<int4 *>(smem + LP_STAGE_OFF) + warp * (LP_GRAN / 2);
     for (int i = tid; i < LP_HIST_BYTES / 4; i += LP_THREADS) H[i] = 0u;
     if (tid == 0) *ctr = 0;
     __syncthreads();
 
-    const int nb = a.nbins;                      // 32, 64, 128 or 256
-    const int mshift = 8 - (31 - __clz(nb));     // rows merged per bin = 1 << mshift
+    const int nb = a.nbins;                      // power of two, 32 <= nb <= LP_ROWS
+    const int mshift = V::ROWLOG - (31 - __clz(nb));   // rows merged per bin = 1 << mshift
     const int M = 1 << mshift;
-    const double M2 = 1729382256910270464.0;     // 1.5 * 2^60: ulp = 256
+    // 1.5 * 2^(52 + ROWLOG): ulp = LP_ROWS
+    const double M2 = (VAR == 0) ? 1729382256910270464.0 : 6917529027641081856.0;
     const bool want_norm = a.out_norm != nullptr;
 
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
@@ -141,6 +211,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
         const long long p0 = (item - curve * ngroups) * LP_GROUP;
         const CurveMeta cm = a.meta[curve];
         const int n = cm.n_valid;
+        if (n < a.n_min || n > a.n_max) continue;      // another launch owns this curve
         const int ntiles = (n + GPFC_TILE - 1) / GPFC_TILE;
 
         // this lane's periods
@@ -152,7 +223,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
             long long j = p0 + r * 32 + lane;
             double x = (j < a.nperiods) ? a.rp[j] : CUDART_NAN;
             valid[r] = (x == x);
-            rp[r] = valid[r] ? x : 256.0;          // dummy period: its columns are never written out
+            rp[r] = valid[r] ? x : (double)LP_ROWS;   // dummy period: its columns are never written out
             if (valid[r]) rpmax = fmax(rpmax, x);
         }
 #pragma unroll
@@ -167,7 +238,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
         // worst tile of the curve: 2^-S <= 2 span_max 2^-32 (or 2^-40)
         const double eq_max = fmax(2.0 * cm.span_max, 1.0 / 256.0) * rpmax;
         const bool fast = (2.0 * (ebase + eq_max) + 2.0 <= 1048576.0) &&
-                          (cm.span_max * rpmax + 512.0 < 1048576.0);
+                          (cm.span_max * rpmax + 2.0 * LP_ROWS < 1048576.0);
 
         if (fast) {
             for (;;) {
@@ -187,9 +258,9 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 double C[LP_R], rps[LP_R];
 #pragma unroll
                 for (int r = 0; r < LP_R; ++r) {
-                    double w = __fma_rd(ti.a, rp[r], M2);       // M2 + 256 * floor(a rp / 256)
+                    double w = __fma_rd(ti.a, rp[r], M2);       // M2 + ROWS * floor(a rp / ROWS)
                     double z = __dsub_rn(w, M2);
-                    double c1 = __fma_rn(ti.a, rp[r], -z);      // (a rp) mod 256, error <= 2^-46
+                    double c1 = __fma_rn(ti.a, rp[r], -z);      // (a rp) mod ROWS, error <= 2^-44
                     C[r] = __dadd_rn(c1, K);
                     rps[r] = __dmul_rn(rp[r], ti.inv_scale);    // exact (power of two)
                 }
@@ -210,17 +281,17 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
 #pragma unroll 1
                         for (int s = 0; s < LP_GRAN / 2; s += 2) {
                             const int4 ra = stage[s], rb = stage[s + 1];
-                            ForR<0>::run((double)(unsigned)ra.x, ra.y, rps, C, lane4, gmin);
-                            ForR<0>::run((double)(unsigned)ra.z, ra.w, rps, C, lane4, gmin);
-                            ForR<0>::run((double)(unsigned)rb.x, rb.y, rps, C, lane4, gmin);
-                            ForR<0>::run((double)(unsigned)rb.z, rb.w, rps, C, lane4, gmin);
+                            ForR<VAR, 0>::run((double)(unsigned)ra.x, ra.y, rps, C, lane4, one, gmin);
+                            ForR<VAR, 0>::run((double)(unsigned)ra.z, ra.w, rps, C, lane4, one, gmin);
+                            ForR<VAR, 0>::run((double)(unsigned)rb.x, rb.y, rps, C, lane4, one, gmin);
+                            ForR<VAR, 0>::run((double)(unsigned)rb.z, rb.w, rps, C, lane4, one, gmin);
                         }
                     } else {
                         const int2 *st2 = reinterpret_cast<const int2 *>(stage);
 #pragma unroll 1
                         for (int s = 0; s < gc; ++s) {
                             const int2 rc = st2[s];
-                            ForR<0>::run((double)(unsigned)rc.x, rc.y, rps, C, lane4, gmin);
+                            ForR<VAR, 0>::run((double)(unsigned)rc.x, rc.y, rps, C, lane4, one, gmin);
                         }
                     }
                 }
@@ -244,10 +315,8 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                                 int kf = __double2hiint(m) & (LP_ROWS - 1);
                                 int ke = exact_bin(us[s], per, LP_ROWS);
                                 if (ke != kf) {
-                                    atomicAdd(&H[hidx(r, kf, 0, lane)], (unsigned)(-rc.y));
-                                    atomicSub(&H[hidx(r, kf, 1, lane)], 1u);
-                                    atomicAdd(&H[hidx(r, ke, 0, lane)], (unsigned)rc.y);
-                                    atomicAdd(&H[hidx(r, ke, 1, lane)], 1u);
+                                    hist_update<VAR>(H, r, kf, lane, rc.y, -1);
+                                    hist_update<VAR>(H, r, ke, lane, rc.y, +1);
                                 }
                             }
                         }
@@ -277,8 +346,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     for (int r = 0; r < LP_R; ++r) {
                         if (valid[r]) {
                             int ke = exact_bin(ui, per[r], LP_ROWS);
-                            atomicAdd(&H[hidx(r, ke, 0, lane)], (unsigned)qi);
-                            atomicAdd(&H[hidx(r, ke, 1, lane)], 1u);
+                            hist_update<VAR>(H, r, ke, lane, qi, +1);
                         }
                     }
                 }
@@ -291,6 +359,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
         // 32-byte sector per output array) for all R period slots.
         const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
         const int octs = nb >> 3;
+        if constexpr (!V::PACKED) {
         {
             // sweep 1: sums and counts out; bin mean m (of the centred flux) back into the
             // bin's first row as an fp64 {lo, hi} (NaN = empty); one-pass moments about the
@@ -373,6 +442,62 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 }
             }
         }
+        } else {
+        {
+            // packed variant, sweep 1: sums and counts out; one-pass moments.  Count words are
+            // shared by rows k and k + 512, so nothing is cleared here unless this is the only
+            // sweep (then the sums are cleared; the counts are cleared below)
+            double s1 = 0.0, s2 = 0.0;
+            int kk = 0;
+            const long long j = p0 + lane;
+            const bool live = j < a.nperiods;
+            const bool ok = live && valid[0];
+            for (int oct = warp; oct < octs && warp < LP_EPI_WARPS; oct += LP_EPI_WARPS) {
+                float fs[8];
+                unsigned fc[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int row0 = (oct * 8 + e) * M;
+                    int S;
+                    unsigned c;
+                    read_bin<VAR>(H, 0, row0, M, lane, S, c);
+                    if (!want_norm)
+                        for (int jj = 0; jj < M; ++jj) H[(row0 + jj) * 32 + lane] = 0u;
+                    if (!ok) {
+                        S = 0;
+                        c = 0;
+                    }
+                    const double sq = __dmul_rn((double)S, inv_scale);
+                    fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
+                    fc[e] = c;
+                    if (want_norm && c > 0) {
+                        const double d = __dsub_rn(__ddiv_rn(sq, (double)c), pivot);
+                        s1 += d;
+                        s2 += __dmul_rn(d, d);
+                        kk += 1;
+                    }
+                }
+                if (live) {
+                    const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
+                    if (a.out_sum) {
+                        float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
+                        o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
+                        o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
+                    }
+                    if (a.out_count) {
+                        uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
+                        o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
+                        o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
+                    }
+                }
+            }
+            if (want_norm && warp < LP_EPI_WARPS) {
+                ps1[warp * LP_GROUP + lane] = s1;
+                ps2[warp * LP_GROUP + lane] = s2;
+                pkk[warp * LP_GROUP + lane] = kk;
+            }
+        }
+        }
         if (want_norm) {
             __syncthreads();
             if (warp < LP_R) {
@@ -396,6 +521,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 st_kk[warp * 32 + lane] = kk;
             }
             __syncthreads();
+            if constexpr (!V::PACKED) {
             // sweep 2: normalised profile out, rows cleared
             for (int oct = warp; oct < octs && warp < LP_EPI_WARPS; oct += LP_EPI_WARPS) {
 #pragma unroll
@@ -424,6 +550,42 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     }
                 }
             }
+                    } else {
+            // packed variant, sweep 2: bin means recomputed from the exact sums and counts,
+            // normalised profile out, sums cleared
+            for (int oct = warp; oct < octs && warp < LP_EPI_WARPS; oct += LP_EPI_WARPS) {
+                const long long j = p0 + lane;
+                const bool live = j < a.nperiods;
+                const double mu = st_mu[lane], isd = st_isd[lane];
+                const double base_o = (live && valid[0] && st_kk[lane] > 0) ? __dadd_rn(mu, center) : 0.0;
+                float fn[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int row0 = (oct * 8 + e) * M;
+                    int S;
+                    unsigned c;
+                    read_bin<VAR>(H, 0, row0, M, lane, S, c);
+                    for (int jj = 0; jj < M; ++jj) H[(row0 + jj) * 32 + lane] = 0u;
+                    double o = base_o;
+                    if (c > 0 && isd > 0.0) {
+                        const double m = __ddiv_rn(__dmul_rn((double)S, inv_scale), (double)c);
+                        o = __dadd_rn(o, __dmul_rn(__dsub_rn(m, mu), isd));
+                    }
+                    fn[e] = (float)o;
+                }
+                if (live) {
+                    float4 *o4 = reinterpret_cast<float4 *>(
+                        a.out_norm + ((curve * a.nperiods + j) * nb) + oct * 8);
+                    o4[0] = make_float4(fn[0], fn[1], fn[2], fn[3]);
+                    o4[1] = make_float4(fn[4], fn[5], fn[6], fn[7]);
+                }
+            }
+            }
+        }
+        if constexpr (V::PACKED) {
+            // every row has been read: clear the packed counts
+            __syncthreads();
+            for (int i = tid; i < 512 * 32; i += LP_THREADS) H[LP_CNT1_OFF / 4 + i] = 0u;
         }
         if (tid == 0) *ctr = 0;
         __syncthreads();   // B: H is zero again, tile counter reset
@@ -434,20 +596,25 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
 
 bool fold_lp_handles(int nbins)
 {
-    return nbins == 32 || nbins == 64 || nbins == 128 || nbins == 256;
+    return nbins == 32 || nbins == 64 || nbins == 128 || nbins == 256 || nbins == 512 ||
+           nbins == 1024;
 }
 
-cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st)
+int fold_lp_rows(int nbins) { return nbins <= 256 ? 256 : 1024; }
+
+template <int VAR>
+static cudaError_t launch_lp_var(FoldArgs a, cudaStream_t st)
 {
     static int state = 0;   // 0 = not initialised, 1 = ready, -1 = shared-memory base differs
+    auto kern = fold_lp_kernel<VAR>;
     if (state == 0) {
-        cudaError_t e = cudaFuncSetAttribute(fold_lp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              LP_SMEM_BYTES);
         if (e != cudaSuccess) return e;
         unsigned *d = nullptr, h = 0;
         e = cudaMalloc(reinterpret_cast<void **>(&d), sizeof(unsigned));
         if (e != cudaSuccess) return e;
-        fold_lp_kernel<<<1, LP_THREADS, LP_SMEM_BYTES, st>>>(a, 0, 0, d);
+        kern<<<1, LP_THREADS, LP_SMEM_BYTES, st>>>(a, 0, 0, d);
         e = cudaMemcpyAsync(&h, d, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         cudaFree(d);
@@ -455,11 +622,25 @@ cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st)
         state = (h == LP_SMEM_BASE) ? 1 : -1;
     }
     if (state < 0) return cudaErrorInvalidConfiguration;   // never seen; reported, not worked around
-    const long long ngroups = (a.nperiods + LP_GROUP - 1) / LP_GROUP;
+    constexpr int GROUP = 32 * LpV<VAR>::R;
+    const long long ngroups = (a.nperiods + GROUP - 1) / GROUP;
     const long long nitems = ngroups * a.ncurves;
     const long long grid = nitems < num_sms() ? nitems : num_sms();
-    fold_lp_kernel<<<(unsigned)grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems, nullptr);
+    kern<<<(unsigned)grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems, nullptr);
     return cudaGetLastError();
+}
+
+cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st)
+{
+    if (a.nbins <= 256) return launch_lp_var<0>(a, st);
+    // packed counts: curves of up to 65,535 valid samples here, longer ones in the generic kernel
+    FoldArgs b = a;
+    b.n_max = LP_PACKED_MAX_N;
+    cudaError_t e = launch_lp_var<1>(b, st);
+    if (e != cudaSuccess) return e;
+    b = a;
+    b.n_min = LP_PACKED_MAX_N + 1;
+    return launch_fold_generic(b, st);
 }
 
 }  // namespace gpfc

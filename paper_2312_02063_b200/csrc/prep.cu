@@ -226,7 +226,7 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
 
 // rp[j] = RN(1/P_j) * rows (exact scaling for power-of-two rows), NaN when the
 // period is not finite and positive.  rows = nbins, or 256 when the lane-period kernel
-// folds at 256 rows and merges adjacent rows at write-out (fold_lp.cu).
+// folds at 256 (or 1024) rows and merges adjacent rows at write-out (fold_lp.cu).
 __global__ void prep_periods_kernel(const double *__restrict__ periods, long long nperiods,
                                     int nbins, double *__restrict__ rp)
 {
@@ -251,7 +251,7 @@ cudaError_t launch_prep(const double *times, const float *flux, const int64_t *o
     if (nperiods > 0) {
         unsigned blocks = (unsigned)((nperiods + 255) / 256);
         prep_periods_kernel<<<blocks, 256, 0, st>>>(periods, nperiods,
-                                                    fold_lp_handles(nbins) ? 256 : nbins, s.rp);
+                                                    fold_lp_handles(nbins) ? fold_lp_rows(nbins) : nbins, s.rp);
     }
     return cudaGetLastError();
 }

@@ -144,6 +144,26 @@ def test_ragged_batch_edge_cases(gp, ref, nbins):
     check(g0, r0)
 
 
+@pytest.mark.parametrize("nbins", [512, 1024])
+def test_packed_counts_long_and_short_curves(gp, ref, nbins):
+    """nbins 512 / 1024 pack two rows' counts in one word (curves of up to 65,535 samples);
+    a longer curve in the same batch is folded by the generic kernel.  Cadence-locked
+    periods put thousands of samples in one bin."""
+    rng = np.random.default_rng(11)
+    dt = workloads.KEPLER_CADENCE_D
+    curves = []
+    for n in (70000, 65535, 65536, 300):
+        t = np.arange(n, dtype=np.float64) * dt
+        f = (rng.integers(-4000, 4000, n).astype(np.float32)) * np.float32(2.0 ** -24)
+        curves.append((t, f, None))
+    periods = np.array([16 * dt, 20 * dt, 0.5, 0.7310371, 1.0, 0.2, np.nan, 25 * dt])
+    w = workloads._pack("packed", -1, curves, 0.2, 1.0, periods.shape[0], nbins, False)
+    g = run_gpu(gp, w, periods)
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
+    check(g, r, exact_sums=True)
+    assert g["count"].max() > 4000           # the degenerate bins are really there
+
+
 def test_guard_band_samples_match_division(gp, ref):
     """Samples that sit exactly on bin edges (t = k P / nb, t = t0) and their
     fp64 neighbours: the reciprocal fast path must fall back to the division."""
@@ -158,7 +178,7 @@ def test_guard_band_samples_match_division(gp, ref):
     t = np.sort(np.concatenate(ts))
     f = rng.integers(-1000, 1000, t.shape[0]).astype(np.float32) * np.float32(2.0 ** -20)
     w = workloads._pack("edges", -1, [(t, f, None)], 0.2, 1.0, periods.shape[0], nb, False)
-    for nbins in (64, 256, 4096):
+    for nbins in (64, 256, 1024, 4096):
         w.nbins = nbins
         g = run_gpu(gp, w, periods)
         r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
