@@ -126,6 +126,20 @@ int gpfc_normalize(const float *sum, const uint32_t *count, int64_t nprofiles, i
                    float *out_norm);
 
 /*
+ * NEXT row: step 4 of the paper's fold, "Fourthly",
+ * Fig. 4(c): merge the nb1 equal-width intermediary bins of each folded profile (e.g. 4096,
+ * from gpfc_fold) into nb2 final bins (e.g. 256) that each contain the same number of points,
+ * scanning left to right and splitting a boundary bin pro rata by count (R18).
+ *   sum, count   device [nprofiles][nb1]   (outputs of gpfc_fold / gpfc_fold_batch)
+ *   out_mean     device fp32 [nprofiles][nb2]  mean flux of each final bin   (may be NULL)
+ *   out_norm     device fp32 [nprofiles][nb2]  the same profile noise-normalised as in
+ *                gpfc_normalize (every final bin counts as non-empty)        (may be NULL)
+ * A profile without points gives zeros.  Arithmetic in fp64.
+ */
+int gpfc_merge_equal_count(const float *sum, const uint32_t *count, int64_t nprofiles, int nb1,
+                           int nb2, float *out_mean, float *out_norm);
+
+/*
  * Batched fold, optionally fused with the normalisation.
  *   times, flux  device, curves stored back to back: curve c is samples
  *                offsets[c] .. offsets[c+1]-1

@@ -28,6 +28,7 @@ EXPORTS = [
     "gpfc_set_workspace", "gpfc_make_period_grid", "gpfc_n_sample", "gpfc_fold",
     "gpfc_normalize", "gpfc_fold_batch", "gpfc_make_period_grid_host",
     "gpfc_fold_batch_host", "gpfc_measure_peaks", "gpfc_profile", "gpfc_profile_read",
+    "gpfc_merge_equal_count",
 ]
 
 
@@ -65,6 +66,7 @@ def lib() -> ctypes.CDLL:
     L.gpfc_fold_batch_host.argtypes = fb
     L.gpfc_measure_peaks.argtypes = [vp]
     L.gpfc_profile.argtypes = [i32]
+    L.gpfc_merge_equal_count.argtypes = [vp, vp, i64, i32, i32, vp, vp]
     L.gpfc_profile_read.argtypes = [vp, vp, vp]
     _lib = L
     return L
@@ -169,6 +171,23 @@ def gpfc_normalize(sum_, count, out_norm=None):
                                 nprof, nb, _dptr(out_norm, torch.float32, "out_norm")),
            "gpfc_normalize")
     return out_norm
+
+
+def gpfc_merge_equal_count(sum_, count, nb2, want=("mean", "norm"), out_mean=None, out_norm=None):
+    """sum_, count: [..., nb1] device tensors -> (mean, norm) [..., nb2] (None if not wanted)."""
+    nb1 = sum_.shape[-1]
+    nprof = sum_.numel() // nb1 if nb1 else 0
+    shape = tuple(sum_.shape[:-1]) + (int(nb2),)
+    if out_mean is None and "mean" in want:
+        out_mean = torch.empty(shape, dtype=torch.float32, device=sum_.device)
+    if out_norm is None and "norm" in want:
+        out_norm = torch.empty(shape, dtype=torch.float32, device=sum_.device)
+    _use_current_stream()
+    _check(lib().gpfc_merge_equal_count(
+        _dptr(sum_, torch.float32, "sum"), _dptr(count, torch.int32, "count"), nprof, nb1, int(nb2),
+        _dptr(out_mean, torch.float32, "out_mean"), _dptr(out_norm, torch.float32, "out_norm")),
+        "gpfc_merge_equal_count")
+    return out_mean, out_norm
 
 
 def gpfc_fold_batch(times, flux, offsets, periods, nbins, t0=None, out_sum=None, out_count=None,

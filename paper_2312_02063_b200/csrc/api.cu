@@ -222,6 +222,21 @@ int gpfc_normalize(const float *sum, const uint32_t *count, int64_t nprofiles, i
     return GPFC_OK;
 }
 
+int gpfc_merge_equal_count(const float *sum, const uint32_t *count, int64_t nprofiles, int nb1,
+                           int nb2, float *out_mean, float *out_norm)
+{
+    if (nprofiles < 0) return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
+    if (nb1 < 1 || nb1 > GPFC_MAX_NBINS || nb2 < 1 || nb2 > GPFC_MAX_NBINS)
+        return fail(GPFC_ERR_UNSUPPORTED, "nb1 and nb2 must be in [1, 4096]%s");
+    if (nprofiles == 0) return GPFC_OK;
+    if (!sum || !count || (!out_mean && !out_norm)) return fail(GPFC_ERR_INVALID_ARG, "NULL pointer%s");
+    cudaError_t e = gpfc::launch_merge(sum, count, nprofiles, nb1, nb2, out_mean, out_norm,
+                                       g_ts.stream);
+    if (e != cudaSuccess) return cuda_fail(e, "merge launch");
+    g_ts.launches += 1;
+    return GPFC_OK;
+}
+
 int gpfc_fold_batch(const double *times, const float *flux, const int64_t *offsets,
                     int64_t ncurves, int64_t n_total, const double *periods, int64_t nperiods,
                     int nbins, const double *t0, float *out_sum, uint32_t *out_count,

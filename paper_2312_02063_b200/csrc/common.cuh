@@ -171,6 +171,8 @@ int fold_lp_rows(int nbins);   // fold resolution of the lane-period kernel (256
 int num_sms();
 cudaError_t launch_normalize(const float *sum, const uint32_t *count, long long nprofiles,
                              int nbins, float *out, cudaStream_t st);
+cudaError_t launch_merge(const float *sum, const uint32_t *count, long long nprofiles, int nb1,
+                         int nb2, float *out_mean, float *out_norm, cudaStream_t st);
 cudaError_t launch_grid(double pmin, double pmax, long long nperiods, int mode_flags,
                         double *out, cudaStream_t st);
 cudaError_t measure_peaks(double *out_host, cudaStream_t st);
