@@ -48,7 +48,9 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (0-4)")
+    ap.add_argument("--config", type=int, default=2,
+                    help="BASELINE.json config index (0-4); 5 = the paper's own two-tier fold "
+                         "(70,000 epochs x 100,000 periods, 4096 -> 256 bins, PAPER.md Table 1)")
     ap.add_argument("--impl", default="gpfc", choices=["gpfc", "reference"])
     ap.add_argument("--curves", type=int, default=0, help="debug: override the number of curves")
     ap.add_argument("--periods", type=int, default=0, help="debug: override the number of periods")
@@ -84,6 +86,12 @@ def max_over_ranks(value, world, device=None):
 
 
 def workload_desc(w, args):
+    if w.config_id == 5:
+        return {"workload": "PAPER.md Table 1 fold: %s" % w.name, "curves": 1,
+                "samples_per_curve": int(w.n_total), "nperiods": int(w.nperiods),
+                "nbins": "4096 intermediary -> 256 equal-count", "outputs": "mean+norm [Np][256]",
+                "grid": "uniform in period, %.1f..%.1f d" % (w.pmin, w.pmax),
+                "l2": "3.3 GB of intermediary sums + counts per step exceed the 126 MB L2"}
     d = {"workload": "BASELINE.json configs[%d] %s" % (w.config_id, w.name),
          "curves": w.ncurves, "samples_per_curve": int(w.n_total // max(w.ncurves, 1)),
          "nperiods": int(w.nperiods), "nbins": int(w.nbins),
@@ -259,9 +267,15 @@ def gpu_arm(args):
     times, flux, offsets = dev(w.times), dev(w.flux), dev(w.offsets)
     shape = (w.ncurves, w.nperiods, w.nbins)
     periods = torch.empty(w.nperiods, dtype=torch.float64, device="cuda")
-    out_norm = torch.empty(shape, dtype=torch.float32, device="cuda")
+    two_tier = (w.config_id == 5)
+    out_norm = None if two_tier else torch.empty(shape, dtype=torch.float32, device="cuda")
     out_sum = out_count = None
-    if not w.fused_normalize:
+    if two_tier:
+        out_sum = torch.empty(shape, dtype=torch.float32, device="cuda")
+        out_count = torch.empty(shape, dtype=torch.int32, device="cuda")
+        mg_mean = torch.empty((w.nperiods, 256), dtype=torch.float32, device="cuda")
+        mg_norm = torch.empty((w.nperiods, 256), dtype=torch.float32, device="cuda")
+    elif not w.fused_normalize:
         out_sum = torch.empty(shape, dtype=torch.float32, device="cuda")
         out_count = torch.empty(shape, dtype=torch.int32, device="cuda")
     ws = torch.empty(gp.gpfc_workspace_bytes(w.ncurves, w.n_total, w.nperiods, w.nbins),
@@ -272,6 +286,8 @@ def gpu_arm(args):
         gp.gpfc_make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode, out=periods)
         gp.gpfc_fold_batch(times, flux, offsets, periods, w.nbins, out_sum=out_sum,
                            out_count=out_count, out_norm=out_norm)
+        if two_tier:
+            gp.gpfc_merge_equal_count(out_sum, out_count, 256, out_mean=mg_mean, out_norm=mg_norm)
 
     def barrier():
         torch.cuda.synchronize()
@@ -312,13 +328,31 @@ def gpu_arm(args):
         torch.cuda.empty_cache()
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
         h_t, h_f, h_o = pin(w.times), pin(w.flux), pin(w.offsets)
-        h_norm = torch.empty(shape, dtype=torch.float32, pin_memory=True)
-        h_sum = h_cnt = None
-        if not w.fused_normalize:
-            h_sum = torch.empty(shape, dtype=torch.float32, pin_memory=True)
-            h_cnt = torch.empty(shape, dtype=torch.int32, pin_memory=True)
+        h_sum = h_cnt = h_norm = None
+        if two_tier:
+            # no host entry point for the two-tier path: the user's calls are the device API
+            # with torch copies (pinned host -> device, merged profiles -> pinned host)
+            h_mean = torch.empty((w.nperiods, 256), dtype=torch.float32, pin_memory=True)
+            h_norm = torch.empty((w.nperiods, 256), dtype=torch.float32, pin_memory=True)
+            d_sum = torch.empty(shape, dtype=torch.float32, device="cuda")
+            d_cnt = torch.empty(shape, dtype=torch.int32, device="cuda")
+        else:
+            h_norm = torch.empty(shape, dtype=torch.float32, pin_memory=True)
+            if not w.fused_normalize:
+                h_sum = torch.empty(shape, dtype=torch.float32, pin_memory=True)
+                h_cnt = torch.empty(shape, dtype=torch.int32, pin_memory=True)
 
         def step_host():
+            if two_tier:
+                dt_, df_, do_ = (h_t.cuda(non_blocking=True), h_f.cuda(non_blocking=True),
+                                 h_o.cuda(non_blocking=True))
+                per = gp.gpfc_make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode)
+                gp.gpfc_fold_batch(dt_, df_, do_, per, w.nbins, out_sum=d_sum, out_count=d_cnt)
+                m_, n_ = gp.gpfc_merge_equal_count(d_sum, d_cnt, 256)
+                h_mean.copy_(m_.view(-1, 256), non_blocking=True)
+                h_norm.copy_(n_.view(-1, 256), non_blocking=True)
+                torch.cuda.synchronize()
+                return
             per = gp.gpfc_make_period_grid_host(w.pmin, w.pmax, w.nperiods, w.grid_mode)
             gp.gpfc_fold_batch_host(h_t, h_f, h_o, per, w.nbins, out_sum=h_sum, out_count=h_cnt,
                                     out_norm=h_norm)
@@ -339,6 +373,10 @@ def gpu_arm(args):
                "h2d_bytes_per_step": int(w.n_total * 12 + w.offsets.nbytes),
                "d2h_bytes_per_step": int(nout * (1 if w.fused_normalize else 3) + w.nperiods * 8),
                "steps": nstep, "api": "gpfc_make_period_grid_host + gpfc_fold_batch_host"}
+        if two_tier:
+            e2e["d2h_bytes_per_step"] = int(2 * w.nperiods * 256 * 4)
+            e2e["api"] = ("torch H2D + gpfc_make_period_grid + gpfc_fold_batch + "
+                          "gpfc_merge_equal_count + torch D2H")
 
     if rank != 0:
         if world > 1:
@@ -355,7 +393,7 @@ def gpu_arm(args):
     roof = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_nominal / 1e9,
             "unit": "G shared-atomic lane-updates/s", "frac": achieved / peak_nominal,
             "traffic": None,
-            "kernel": "fold_lp_kernel" if w.nbins in (32, 64, 128, 256) else "fold_cols_kernel", "kernel_ms": fold_ms,
+            "kernel": "fold_lp_kernel" if w.nbins <= 1024 else "fold_cols_kernel", "kernel_ms": fold_ms,
             "peak_source": "derived: 148 SMs x 32 lanes/clk x %.0f MHz" % sm_max,
             "hbm_bound": {"algorithmic_bytes": out_bytes + w.n_total * 12.0,
                           "achieved_gbs": (out_bytes + w.n_total * 12.0) / (fold_ms * 1e-3) / 1e9}}
@@ -376,8 +414,17 @@ def gpu_arm(args):
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": workload_desc(w, args), "clocks": clocks, "roofline": roof,
            "gpu_launches": int(prof["kernel_launches"])}
+    if two_tier:
+        # the paper's profiled fold, same workload, RTX 3090 Ti (context, not target)
+        out["vs_baseline"] = value / (70000.0 * 100000.0 / 4.32)
+        out["paper"] = {"workload_s_paper_total": 5.00, "workload_s_paper_gpu_kernels_plus_device_memory": 4.32,
+                        "workload_s_here_device": ms / args.steps * 1e-3,
+                        "vs_baseline_denominator": "7e9 point-periods / 4.32 s (Table 1: 0.66 s kernels "
+                        "+ 3.66 s device memory), PAPER.md:130-131", "hardware_paper": "RTX 3090 Ti"}
     if e2e:
         out["e2e"] = e2e
+        if two_tier:
+            out["paper"]["workload_s_here_e2e"] = 70000.0 * 100000.0 / e2e["value"]
     if not args.no_cpu:
         periods_host = periods.cpu().numpy()
         out["cpu_baseline"] = cpu_baseline(w, periods_host)

@@ -183,7 +183,27 @@ def config4(ncurves=4096, nperiods=50_000, first_curve=0):
     return _pack("config4_tess_batch_fused", 4, curves, 0.2, 1.0, nperiods, 128, True)
 
 
-CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
+def paper_fold(nperiods=100_000, n=70_000):
+    """The paper's own fold workload (Table 1 :125-142): one
+    Kepler-like curve of 70,000 epochs (profiled case), 100,000 trial periods uniform IN PERIOD
+    over [0.2, 1.0] d (0.69 s granularity), 4096 intermediary bins merged to 256 equal-count
+    bins.  nbins here is the intermediary count; bench.py merges to 256."""
+    rng = np.random.default_rng([5, 0])
+    nslots = int(round(n / 0.94))
+    keep = np.sort(rng.choice(nslots, size=n, replace=False))
+    t = keep.astype(np.float64) * KEPLER_CADENCE_D
+    p0 = float(rng.uniform(0.2, 1.0))
+    box = dict(p0=p0, depth=1e-4, dur=0.03)
+    epoch = float(rng.uniform(0.0, p0))
+    f = 1.0 + rng.normal(0.0, 3e-4, size=n)
+    f = f - box["depth"] * _box_mask(t, p0, box["dur"], epoch)
+    w = _pack("paper_fold_two_tier", 5, [(t, _finish(f), dict(box, epoch=epoch))], 0.2, 1.0,
+              nperiods, 4096, False)
+    w.grid_mode = GRID_UNIFORM_PERIOD
+    return w
+
+
+CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4, 5: paper_fold}
 
 
 def make(config_id: int, **kw) -> Workload:
