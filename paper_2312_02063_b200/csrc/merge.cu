@@ -6,9 +6,10 @@
 // the last bin) inside the first fine bin k with C(k) >= target_b:
 //     Scum_b  = S(k-1) + ((target_b - C(k-1)) / count[k]) * sum[k]
 //     out_sum[b] = Scum_b - Scum_{b-1},  out_mean[b] = out_sum[b] / (N / nb2)
-// One warp per profile: lane l owns nb1/32 consecutive fine bins, a warp scan gives the
-// cumulative count and sum at the start of its chunk, and the lane emits the boundaries that
-// fall inside its bins.  fp64 throughout, every operation rounded once (no FMA).
+// One warp per profile: the profile is staged in shared memory with coalesced loads (padded
+// by one word per lane chunk, so the per-lane walks below are bank-conflict-free); lane l owns
+// nb1/32 consecutive fine bins, a warp scan gives the cumulative count and sum at the start of
+// its chunk, and the lane emits the boundaries that fall inside its bins.  fp64 throughout, every operation rounded once (no FMA).
 // Optionally the merged profile is noise-normalised in the same pass.
 #include "common.cuh"
 
@@ -16,7 +17,8 @@ namespace gpfc {
 
 namespace {
 
-constexpr int MERGE_THREADS = 256;   // fewer when nb2 is large (8 (nb2 + 1) bytes per warp)
+constexpr int MERGE_THREADS = 512;   // fewer when nb2 is large (8 (nb2 + 1) bytes per warp)
+constexpr int MERGE_SEG = 1024;      // fine bins staged per pass (per warp: 8.4 KB)
 
 __global__ void __launch_bounds__(MERGE_THREADS)
 merge_equal_count_kernel(const float *__restrict__ sum, const uint32_t *__restrict__ count,
@@ -25,34 +27,36 @@ merge_equal_count_kernel(const float *__restrict__ sum, const uint32_t *__restri
 {
     extern __shared__ __align__(16) unsigned char merge_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double *scum = reinterpret_cast<double *>(merge_smem) + (size_t)warp * (nb2 + 1);
-    const int chunk = (nb1 + 31) / 32;
     const int nwarps = blockDim.x >> 5;
+    const int seg = min(nb1, MERGE_SEG);
+    const int chunk = (seg + 31) / 32;                    // bins per lane and segment
+    const int pad = (chunk & 1) ? 0 : 1;                  // lane stride chunk + pad is odd
+    const unsigned magic = (chunk > 1) ? (unsigned)((4294967296ull + chunk - 1) / chunk) : 0u;
+    const int padded = seg + 32;
+    double *scum = reinterpret_cast<double *>(merge_smem) + (size_t)warp * (nb2 + 1);
+    float *fs = reinterpret_cast<float *>(reinterpret_cast<double *>(merge_smem) +
+                                          (size_t)nwarps * (nb2 + 1)) + (size_t)warp * 2 * padded;
+    uint32_t *fc = reinterpret_cast<uint32_t *>(fs + padded);
     for (long long prof = (long long)blockIdx.x * nwarps + warp; prof < nprofiles;
          prof += (long long)gridDim.x * nwarps) {
-        const float *s = sum + prof * nb1;
-        const uint32_t *c = count + prof * nb1;
-        const int k0 = min(nb1, lane * chunk), k1 = min(nb1, k0 + chunk);
-        // chunk totals -> exclusive warp scan
-        double cs = 0.0, ss = 0.0;
-        for (int k = k0; k < k1; ++k) {
-            cs += (double)c[k];
-            ss += (double)s[k];
-        }
-        double cpre = cs, spre = ss;
+        const float *gs = sum + prof * nb1;
+        const uint32_t *gc = count + prof * nb1;
+        // total number of points of the profile
+        unsigned tot_i = 0;
+        for (int kb = 0; kb < nb1; kb += 256) {
+            unsigned v[8];
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            double a = __shfl_up_sync(0xffffffffu, cpre, o);
-            double b = __shfl_up_sync(0xffffffffu, spre, o);
-            if (lane >= o) {
-                cpre += a;
-                spre += b;
+            for (int j = 0; j < 8; ++j) {
+                const int k = kb + j * 32 + lane;
+                v[j] = (k < nb1) ? gc[k] : 0u;
             }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) tot_i += v[j];
         }
-        const double total = __shfl_sync(0xffffffffu, cpre, 31);
-        double cb = cpre - cs, sb = spre - ss;      // cumulative count / sum before fine bin k0
-        __syncwarp();
-        if (!(total > 0.0)) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) tot_i += __shfl_xor_sync(0xffffffffu, tot_i, o);
+        const double total = (double)tot_i;
+        if (tot_i == 0u) {
             for (int b = lane; b < nb2; b += 32) {
                 if (out_mean) out_mean[prof * nb2 + b] = 0.f;
                 if (out_norm) out_norm[prof * nb2 + b] = 0.f;
@@ -60,25 +64,90 @@ merge_equal_count_kernel(const float *__restrict__ sum, const uint32_t *__restri
             continue;
         }
         const double per = __ddiv_rn(total, (double)nb2);
-        // first boundary whose target lies beyond the points before this chunk
-        int b = (int)floor(__ddiv_rn(cb, per)) - 1;
-        if (b < 0) b = 0;
-        while (b < nb2 && !(((b == nb2 - 1) ? total : __dmul_rn(per, (double)(b + 1))) > cb)) ++b;
-        if (lane == 0) b = 0;
-        for (int k = k0; k < k1; ++k) {
-            const double ck = (double)c[k], sk = (double)s[k];
-            const double ca = cb + ck;
-            const bool last = (k == nb1 - 1);
-            while (b < nb2) {
-                const double target = (b == nb2 - 1) ? total : __dmul_rn(per, (double)(b + 1));
-                if (!last && ca < target) break;            // boundary lies in a later bin
-                double frac = (ck > 0.0) ? __ddiv_rn(__dsub_rn(target, cb), ck) : 0.0;
-                frac = fmin(fmax(frac, 0.0), 1.0);
-                scum[b + 1] = __dadd_rn(sb, __dmul_rn(frac, sk));
-                ++b;
+        unsigned cum_c = 0;        // points before the current segment
+        double cum_s = 0.0;        // flux before the current segment
+        for (int s0 = 0; s0 < nb1; s0 += seg) {
+            const int sn = min(seg, nb1 - s0);
+            __syncwarp();
+            // stage the segment: 8 independent coalesced loads in flight per array
+            for (int kb = 0; kb < sn; kb += 256) {
+                float vs[8];
+                uint32_t vc[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int k = kb + j * 32 + lane;
+                    vs[j] = (k < sn) ? gs[s0 + k] : 0.f;
+                    vc[j] = (k < sn) ? gc[s0 + k] : 0u;
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int k = kb + j * 32 + lane;
+                    if (k < sn) {
+                        const int q = (chunk > 1) ? (int)__umulhi((unsigned)k, magic) : k;   // k / chunk
+                        fs[k + pad * q] = vs[j];
+                        fc[k + pad * q] = vc[j];
+                    }
+                }
             }
-            cb = ca;
-            sb += sk;
+            __syncwarp();
+            const int k0 = min(sn, lane * chunk), k1 = min(sn, k0 + chunk);
+            const float *s = fs + pad * lane;            // s[k] for k in [k0, k1)
+            const uint32_t *c = fc + pad * lane;
+            // chunk totals -> exclusive warp scan
+            unsigned cs = 0;
+            double ss = 0.0;
+            for (int k = k0; k < k1; ++k) {
+                cs += c[k];
+                ss += (double)s[k];
+            }
+            unsigned cpre = cs;
+            double spre = ss;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                unsigned a = __shfl_up_sync(0xffffffffu, cpre, o);
+                double b = __shfl_up_sync(0xffffffffu, spre, o);
+                if (lane >= o) {
+                    cpre += a;
+                    spre += b;
+                }
+            }
+            const unsigned seg_c = __shfl_sync(0xffffffffu, cpre, 31);
+            const double seg_s = __shfl_sync(0xffffffffu, spre, 31);
+            unsigned cbi = cum_c + (cpre - cs);           // points before fine bin s0 + k0
+            double sb = cum_s + (spre - ss);              // flux before it
+            // first boundary whose target lies beyond the points before this chunk
+            const double cbd0 = (double)cbi;
+            int b = (int)floor(__ddiv_rn(cbd0, per)) - 1;
+            if (b < 0) b = 0;
+            while (b < nb2 && !(((b == nb2 - 1) ? total : __dmul_rn(per, (double)(b + 1))) > cbd0)) ++b;
+            if (cbi == 0u) b = 0;
+            // walk this lane's bins.  Counts are integers, so "C(k) >= target" is the integer
+            // test C(k) > thr with thr = ceil(target) - 1; fp64 only when a boundary is emitted.
+            double target = (b < nb2) ? ((b == nb2 - 1) ? total : __dmul_rn(per, (double)(b + 1))) : 0.0;
+            unsigned thr = (b < nb2) ? (unsigned)ceil(target) - 1u : 0xffffffffu;
+            for (int k = k0; k < k1; ++k) {
+                const unsigned cki = c[k];
+                const double sk = (double)s[k];
+                const unsigned cai = cbi + cki;
+                const bool last = (s0 + k == nb1 - 1);
+                if (b < nb2 && (last || cai > thr)) {
+                    const double ck = (double)cki, cbd = (double)cbi;
+                    do {
+                        double frac = (cki > 0u) ? __ddiv_rn(__dsub_rn(target, cbd), ck) : 0.0;
+                        frac = fmin(fmax(frac, 0.0), 1.0);
+                        scum[b + 1] = __dadd_rn(sb, __dmul_rn(frac, sk));
+                        ++b;
+                        if (b < nb2) {
+                            target = (b == nb2 - 1) ? total : __dmul_rn(per, (double)(b + 1));
+                            thr = (unsigned)ceil(target) - 1u;
+                        }
+                    } while (b < nb2 && (last || cai > thr));
+                }
+                cbi = cai;
+                sb += sk;
+            }
+            cum_c += seg_c;
+            cum_s += seg_s;
         }
         if (lane == 0) scum[0] = 0.0;
         __syncwarp();
@@ -117,10 +186,12 @@ cudaError_t launch_merge(const float *sum, const uint32_t *count, long long npro
 {
     if (nprofiles <= 0) return cudaSuccess;
     int warps = MERGE_THREADS / 32;
-    while (warps > 1 && (size_t)warps * (nb2 + 1) * sizeof(double) > 96 * 1024) warps >>= 1;
+    const int seg = nb1 < MERGE_SEG ? nb1 : MERGE_SEG;
+    const size_t per_warp = (size_t)(nb2 + 1) * sizeof(double) + (size_t)2 * (seg + 32) * 4;
+    while (warps > 1 && (size_t)warps * per_warp > 200 * 1024) --warps;
     long long blocks = (nprofiles + warps - 1) / warps;
     if (blocks > 148LL * 16) blocks = 148LL * 16;
-    size_t smem = (size_t)warps * (nb2 + 1) * sizeof(double);
+    size_t smem = (size_t)warps * per_warp;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(merge_equal_count_kernel,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
