@@ -72,6 +72,7 @@ constexpr int LP_KK_OFF = LP_ISD_OFF + LP_GROUP_MAX * 8;                   // in
 constexpr int LP_CTR_OFF = LP_KK_OFF + LP_GROUP_MAX * 4;
 constexpr int LP_SMEM_BYTES = LP_CTR_OFF + 16;
 static_assert(LP_SMEM_BYTES <= 227 * 1024, "shared memory budget");
+static_assert(GPFC_TILE == 2 * LP_GRAN, "half-tile work units are one staging granule");
 static_assert(LP_WARPS * LP_GRAN * 8 <= LP_MU_OFF - LP_STAGE_OFF, "staging fits in the scratch");
 
 // shared-memory reductions with an immediate offset: ATOMS.ADD / ATOMS.POPC.INC
@@ -128,6 +129,19 @@ __device__ __forceinline__ void read_bin(const unsigned *H, int r, int row0, int
 }
 
 // one point-period of the fast path for period slot r (compile-time)
+// sq / c for a count c in [1, 2^32): reciprocal from an fp32 seed + two Newton steps
+// (relative error < 2^-49), then one residual correction.  The result is exact whenever the
+// quotient is representable (what the flat-profile test needs) and within 1 ulp otherwise.
+__device__ __forceinline__ double div_by_count(double sq, unsigned c)
+{
+    const double cd = (double)c;
+    double r = (double)__frcp_rn((float)c);
+    r = __fma_rn(__fma_rn(-cd, r, 1.0), r, r);
+    r = __fma_rn(__fma_rn(-cd, r, 1.0), r, r);
+    const double q0 = __dmul_rn(sq, r);
+    return __fma_rn(__fma_rn(-q0, cd, sq), r, q0);
+}
+
 // the constant 1 in a register the compiler cannot fold, so that (t7 & 0x10000) | 1 is ONE LOP3
 __device__ __forceinline__ unsigned opaque_one()
 {
@@ -241,13 +255,20 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                           (cm.span_max * rpmax + 2.0 * LP_ROWS < 1048576.0);
 
         if (fast) {
+            // work units: whole anchor tiles first, then the last 2 * LP_WARPS tiles in halves
+            // (one staging granule each), so that the warps reach the barrier closer together
+            const int nfull = max(0, ntiles - 2 * LP_WARPS);
+            const int nunits = nfull + 2 * (ntiles - nfull);
             for (;;) {
-                int t = 0;
-                if (lane == 0) t = atomicAdd(ctr, 1);
-                t = __shfl_sync(0xffffffffu, t, 0);
-                if (t >= ntiles) break;
-                const int base = t * GPFC_TILE;
-                const int cnt = min(GPFC_TILE, n - base);
+                int u = 0;
+                if (lane == 0) u = atomicAdd(ctr, 1);
+                u = __shfl_sync(0xffffffffu, u, 0);
+                if (u >= nunits) break;
+                const int t = (u < nfull) ? u : nfull + ((u - nfull) >> 1);
+                const int half = (u < nfull) ? 0 : ((u - nfull) & 1);
+                const int base = t * GPFC_TILE + half * LP_GRAN;
+                const int cnt = min((u < nfull) ? GPFC_TILE : LP_GRAN, n - base);
+                if (cnt <= 0) continue;
                 const TileInfo ti = a.tiles[cm.tile0 + t];
                 // D = smallest power of two >= need (>= 16): exponent trick, need = f 2^e, f < 1
                 const double need = 2.0 * (ebase + ti.inv_scale * rpmax * 4294967296.0) + 2.0;
@@ -363,83 +384,75 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
         {
             // sweep 1: sums and counts out; bin mean m (of the centred flux) back into the
             // bin's first row as an fp64 {lo, hi} (NaN = empty); one-pass moments about the
-            // curve mean (exactly zero for a flat profile)
-            double s1[LP_R], s2[LP_R];
-            int kk[LP_R];
+            // curve mean (exactly zero for a flat profile).  Warp group g = warp / WPR takes
+            // period slot r = g, its WPR warps split the octets of bins.
+            constexpr int WPR = LP_WARPS / LP_R;
+            static_assert(LP_WARPS % LP_R == 0, "warps per period slot");
+            const int r = warp / WPR, wr = warp - r * WPR;
+            double s1 = 0.0, s2 = 0.0;
+            int kk = 0;
+            const long long j = p0 + r * 32 + lane;
+            const bool live = j < a.nperiods;
+            bool ok = false;
 #pragma unroll
-            for (int r = 0; r < LP_R; ++r) {
-                s1[r] = 0.0;
-                s2[r] = 0.0;
-                kk[r] = 0;
-            }
-            for (int oct = warp; oct < octs && warp < LP_EPI_WARPS; oct += LP_EPI_WARPS) {
+            for (int rr = 0; rr < LP_R; ++rr)
+                if (rr == r) ok = live && valid[rr];
+            unsigned *Hr = H + r * (LP_ROWS * 64) + lane;
+            for (int oct = wr; oct < octs; oct += WPR) {
+                float fs[8];
+                unsigned fc[8];
 #pragma unroll
-                for (int r = 0; r < LP_R; ++r) {
-                    const long long j = p0 + r * 32 + lane;
-                    const bool live = j < a.nperiods;
-                    const bool ok = live && valid[r];
-                    float fs[8];
-                    unsigned fc[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        const int row0 = (oct * 8 + e) * M;
-                        int S = 0;
-                        unsigned c = 0;
-                        for (int jj = 0; jj < M; ++jj) {
-                            const int i0 = hidx(r, row0 + jj, 0, lane);
-                            S += (int)H[i0];
-                            c += H[i0 + 32];
-                            if (jj > 0) {
-                                H[i0] = 0u;
-                                H[i0 + 32] = 0u;
-                            }
-                        }
-                        if (!ok) {
-                            S = 0;
-                            c = 0;
-                        }
-                        const double sq = __dmul_rn((double)S, inv_scale);
-                        fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
-                        fc[e] = c;
-                        const int i0 = hidx(r, row0, 0, lane);
-                        if (want_norm) {
-                            double m = CUDART_NAN;
-                            if (c > 0) {
-                                m = __ddiv_rn(sq, (double)c);
-                                const double d = __dsub_rn(m, pivot);
-                                s1[r] += d;
-                                s2[r] += __dmul_rn(d, d);
-                                kk[r] += 1;
-                            }
-                            H[i0] = (unsigned)__double2loint(m);
-                            H[i0 + 32] = (unsigned)__double2hiint(m);
-                        } else {
-                            H[i0] = 0u;
-                            H[i0 + 32] = 0u;
-                        }
+                for (int e = 0; e < 8; ++e) {
+                    unsigned *h0 = Hr + (oct * 8 + e) * M * 64;
+                    int S = (int)h0[0];
+                    unsigned c = h0[32];
+                    for (int jj = 1; jj < M; ++jj) {
+                        S += (int)h0[jj * 64];
+                        c += h0[jj * 64 + 32];
+                        h0[jj * 64] = 0u;
+                        h0[jj * 64 + 32] = 0u;
                     }
-                    if (live) {
-                        const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
-                        if (a.out_sum) {
-                            float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
-                            o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
-                            o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
+                    if (!ok) {
+                        S = 0;
+                        c = 0;
+                    }
+                    const double sq = __dmul_rn((double)S, inv_scale);
+                    fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
+                    fc[e] = c;
+                    if (want_norm) {
+                        double m = CUDART_NAN;
+                        if (c > 0) {
+                            m = div_by_count(sq, c);
+                            const double d = __dsub_rn(m, pivot);
+                            s1 += d;
+                            s2 += __dmul_rn(d, d);
+                            kk += 1;
                         }
-                        if (a.out_count) {
-                            uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
-                            o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
-                            o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
-                        }
+                        h0[0] = (unsigned)__double2loint(m);
+                        h0[32] = (unsigned)__double2hiint(m);
+                    } else {
+                        h0[0] = 0u;
+                        h0[32] = 0u;
+                    }
+                }
+                if (live) {
+                    const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
+                    if (a.out_sum) {
+                        float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
+                        o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
+                        o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
+                    }
+                    if (a.out_count) {
+                        uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
+                        o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
+                        o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
                     }
                 }
             }
-            if (want_norm && warp < LP_EPI_WARPS) {
-#pragma unroll
-                for (int r = 0; r < LP_R; ++r) {
-                    ps1[warp * LP_GROUP + r * 32 + lane] = s1[r];
-                    ps2[warp * LP_GROUP + r * 32 + lane] = s2[r];
-                    pkk[warp * LP_GROUP + r * 32 + lane] = kk[r];
-                }
+            if (want_norm) {
+                ps1[wr * LP_GROUP + r * 32 + lane] = s1;
+                ps2[wr * LP_GROUP + r * 32 + lane] = s2;
+                pkk[wr * LP_GROUP + r * 32 + lane] = kk;
             }
         }
         } else {
@@ -503,7 +516,8 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
             if (warp < LP_R) {
                 double s1 = 0.0, s2 = 0.0;
                 int kk = 0;
-                for (int w = 0; w < LP_EPI_WARPS; ++w) {   // fixed order: deterministic
+                constexpr int NPART = V::PACKED ? LP_EPI_WARPS : LP_WARPS / LP_R;
+                for (int w = 0; w < NPART; ++w) {          // fixed order: deterministic
                     s1 += ps1[w * LP_GROUP + warp * 32 + lane];
                     s2 += ps2[w * LP_GROUP + warp * 32 + lane];
                     kk += pkk[w * LP_GROUP + warp * 32 + lane];
@@ -522,22 +536,27 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
             }
             __syncthreads();
             if constexpr (!V::PACKED) {
-            // sweep 2: normalised profile out, rows cleared
-            for (int oct = warp; oct < octs && warp < LP_EPI_WARPS; oct += LP_EPI_WARPS) {
+            // sweep 2: normalised profile out, rows cleared (same split as sweep 1)
+            {
+                constexpr int WPR = LP_WARPS / LP_R;
+                const int r = warp / WPR, wr = warp - r * WPR;
+                const long long j = p0 + r * 32 + lane;
+                const bool live = j < a.nperiods;
+                bool okr = false;
 #pragma unroll
-                for (int r = 0; r < LP_R; ++r) {
-                    const long long j = p0 + r * 32 + lane;
-                    const bool live = j < a.nperiods;
-                    const double mu = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
-                    const double base_o = (live && valid[r] && st_kk[r * 32 + lane] > 0)
-                                              ? __dadd_rn(mu, center) : 0.0;
+                for (int rr = 0; rr < LP_R; ++rr)
+                    if (rr == r) okr = valid[rr];
+                const double mu = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
+                const double base_o = (live && okr && st_kk[r * 32 + lane] > 0) ? __dadd_rn(mu, center) : 0.0;
+                unsigned *Hr = H + r * (LP_ROWS * 64) + lane;
+                for (int oct = wr; oct < octs; oct += WPR) {
                     float fn[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
-                        const int i0 = hidx(r, (oct * 8 + e) * M, 0, lane);
-                        const double m = __hiloint2double((int)H[i0 + 32], (int)H[i0]);
-                        H[i0] = 0u;
-                        H[i0 + 32] = 0u;
+                        unsigned *h0 = Hr + (oct * 8 + e) * M * 64;
+                        const double m = __hiloint2double((int)h0[32], (int)h0[0]);
+                        h0[0] = 0u;
+                        h0[32] = 0u;
                         double o = base_o;
                         if (m == m && isd > 0.0) o = __dadd_rn(o, __dmul_rn(__dsub_rn(m, mu), isd));
                         fn[e] = (float)o;
@@ -550,7 +569,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     }
                 }
             }
-                    } else {
+            } else {
             // packed variant, sweep 2: bin means recomputed from the exact sums and counts,
             // normalised profile out, sums cleared
             for (int oct = warp; oct < octs && warp < LP_EPI_WARPS; oct += LP_EPI_WARPS) {
