@@ -36,7 +36,7 @@ namespace {
 
 constexpr int LP_THREADS = 768;
 constexpr int LP_WARPS = LP_THREADS / 32;
-constexpr int LP_EPI_WARPS = 16;              // warps that run the epilogue sweeps
+constexpr int LP_EPI_WARPS = 16;              // sizes the statistics partials: (LP_WARPS / R) * 32 R <= 16 * 96
 constexpr int LP_GRAN = 64;                   // samples per staging granule
 constexpr unsigned LP_SMEM_BASE = 0x400;      // shared-window address of dynamic shared memory
 
@@ -465,7 +465,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
             const long long j = p0 + lane;
             const bool live = j < a.nperiods;
             const bool ok = live && valid[0];
-            for (int oct = warp; oct < octs && warp < LP_EPI_WARPS; oct += LP_EPI_WARPS) {
+            for (int oct = warp; oct < octs; oct += LP_WARPS) {
                 float fs[8];
                 unsigned fc[8];
 #pragma unroll
@@ -484,7 +484,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
                     fc[e] = c;
                     if (want_norm && c > 0) {
-                        const double d = __dsub_rn(__ddiv_rn(sq, (double)c), pivot);
+                        const double d = __dsub_rn(div_by_count(sq, c), pivot);
                         s1 += d;
                         s2 += __dmul_rn(d, d);
                         kk += 1;
@@ -504,7 +504,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     }
                 }
             }
-            if (want_norm && warp < LP_EPI_WARPS) {
+            if (want_norm) {
                 ps1[warp * LP_GROUP + lane] = s1;
                 ps2[warp * LP_GROUP + lane] = s2;
                 pkk[warp * LP_GROUP + lane] = kk;
@@ -516,7 +516,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
             if (warp < LP_R) {
                 double s1 = 0.0, s2 = 0.0;
                 int kk = 0;
-                constexpr int NPART = V::PACKED ? LP_EPI_WARPS : LP_WARPS / LP_R;
+                constexpr int NPART = LP_WARPS / LP_R;
                 for (int w = 0; w < NPART; ++w) {          // fixed order: deterministic
                     s1 += ps1[w * LP_GROUP + warp * 32 + lane];
                     s2 += ps2[w * LP_GROUP + warp * 32 + lane];
@@ -572,7 +572,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
             } else {
             // packed variant, sweep 2: bin means recomputed from the exact sums and counts,
             // normalised profile out, sums cleared
-            for (int oct = warp; oct < octs && warp < LP_EPI_WARPS; oct += LP_EPI_WARPS) {
+            for (int oct = warp; oct < octs; oct += LP_WARPS) {
                 const long long j = p0 + lane;
                 const bool live = j < a.nperiods;
                 const double mu = st_mu[lane], isd = st_isd[lane];
@@ -587,7 +587,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     for (int jj = 0; jj < M; ++jj) H[(row0 + jj) * 32 + lane] = 0u;
                     double o = base_o;
                     if (c > 0 && isd > 0.0) {
-                        const double m = __ddiv_rn(__dmul_rn((double)S, inv_scale), (double)c);
+                        const double m = div_by_count(__dmul_rn((double)S, inv_scale), c);
                         o = __dadd_rn(o, __dmul_rn(__dsub_rn(m, mu), isd));
                     }
                     fn[e] = (float)o;
