@@ -404,6 +404,14 @@ def gpu_arm(args):
     except (OSError, KeyError, ValueError):
         roof["hbm_bound"]["peak_gbs"] = 6650.0
         roof["hbm_bound"]["peak_source"] = "fallback"
+    try:   # DRAM bytes per launch from the committed ncu capture of this workload, if any
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r1_traffic.json"))).get(w.name)
+        if tj and (tj["curves"], tj["nperiods"], tj["nbins"]) == (w.ncurves, w.nperiods, w.nbins):
+            roof["traffic"] = tj["traffic_bytes"]
+            roof["traffic_source"] = "profiles/r1_traffic.json (ncu --set full, commit %s)" % tj["commit"]
+            roof["algorithmic_bytes"] = out_bytes + w.n_total * 12.0
+    except (OSError, KeyError, ValueError):
+        pass
     if peaks:
         roof["measured_peak"] = peaks["smem_atomic_lane_updates_per_s"] / 1e9
         roof["frac_of_measured"] = achieved / peaks["smem_atomic_lane_updates_per_s"]
