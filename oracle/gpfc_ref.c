@@ -112,11 +112,15 @@ int gpfc_ref_make_period_grid(double pmin, double pmax, int64_t nperiods,
  *                                    negative x rounds up in x + 1
  *   k   = trunc(phi * nb)            R4: half-open bins [k/nb, (k+1)/nb)
  *   k   = nb-1 if k >= nb            R4: phi == 1.0 belongs to the last bin
+ * R20: if u / P is not finite (a denormal-small P) the sample has no phase: -1, and the
+ * fold skips it like a non-finite sample (R13).
  */
 static int64_t bin_of(double t, double t0, double period, int nb)
 {
     double u = t - t0;
     double x = u / period;
+    if (!isfinite(x))
+        return -1;   /* R20: the quotient overflows (period far below |u| / DBL_MAX): skip */
     double phi = x - floor(x);
     double scaled = phi * (double)nb;
     int64_t k = (int64_t)scaled;
@@ -174,6 +178,8 @@ int gpfc_ref_fold(const double *times, const float *flux, int64_t n,
                 if (!isfinite(times[i]) || !isfinite(flux[i]))
                     continue;
                 int64_t k = bin_of(times[i], t0, period, nbins);
+                if (k < 0)
+                    continue;
                 s[k] += (double)flux[i];
                 c[k] += 1;
             }

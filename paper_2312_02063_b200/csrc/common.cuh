@@ -63,12 +63,13 @@ struct FoldArgs {
     int n_min, n_max;   // a launch handles the curves with n_min <= n_valid <= n_max
 };
 
-// ---- exact bin of one sample: the formula of include/gpfc.h, every operation
+// ---- exact bin of one sample (-1 = skip the sample, reading R20): the formula of include/gpfc.h, every operation
 // rounded once (intrinsics, so nothing can be contracted into an FMA).
 // PAPER.md:111 "First", "Secondly".
 __device__ __forceinline__ int exact_bin(double u, double period, int nbins)
 {
     double x = __ddiv_rn(u, period);
+    if (!(fabs(x) < CUDART_INF)) return -1;   // R20: u / P overflows -> the sample is skipped
     double phi = __dsub_rn(x, floor(x));
     double scaled = __dmul_rn(phi, (double)nbins);
     long long k = (long long)scaled;   // truncation; scaled >= 0

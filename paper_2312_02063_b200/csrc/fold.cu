@@ -152,11 +152,13 @@ fold_cols_kernel(FoldArgs a, long long ngroups, long long nitems)
                                 int ke = exact_bin(uu[k], a.periods[p0 + p], NB);
                                 if (ke != kf) {
                                     int *hf = H + p * 2 * HW + kf * COLS + col;
-                                    int *he = H + p * 2 * HW + ke * COLS + col;
                                     atomicAdd(hf, -qq[k]);
                                     atomicSub(reinterpret_cast<unsigned *>(hf + HW), 1u);
-                                    atomicAdd(he, qq[k]);
-                                    atomicAdd(reinterpret_cast<unsigned *>(he + HW), 1u);
+                                    if (ke >= 0) {
+                                        int *he = H + p * 2 * HW + ke * COLS + col;
+                                        atomicAdd(he, qq[k]);
+                                        atomicAdd(reinterpret_cast<unsigned *>(he + HW), 1u);
+                                    }
                                 }
                             }
                         }
@@ -185,6 +187,7 @@ fold_cols_kernel(FoldArgs a, long long ngroups, long long nitems)
                         for (int p = 0; p < PB; ++p) {
                             if (period_ok(per[p])) {
                                 int ke = exact_bin(ui, per[p], NB);
+                                if (ke < 0) continue;
                                 int *he = H + p * 2 * HW + ke * COLS + col;
                                 atomicAdd(he, qi);
                                 atomicAdd(reinterpret_cast<unsigned *>(he + HW), 1u);
@@ -261,6 +264,7 @@ fold_generic_kernel(FoldArgs a, long long nitems)
             const int *__restrict__ q = a.q + m.start;
             for (int i = tid; i < m.n_valid; i += GEN_THREADS) {
                 int ke = exact_bin(u[i], per, nb);
+                if (ke < 0) continue;
                 unsigned *slot = reinterpret_cast<unsigned *>(R + ke);
                 atomicAdd(slot, (unsigned)q[i]);
                 atomicAdd(slot + 1, 1u);

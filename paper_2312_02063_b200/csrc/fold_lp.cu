@@ -337,7 +337,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                                 int ke = exact_bin(us[s], per, LP_ROWS);
                                 if (ke != kf) {
                                     hist_update<VAR>(H, r, kf, lane, rc.y, -1);
-                                    hist_update<VAR>(H, r, ke, lane, rc.y, +1);
+                                    if (ke >= 0) hist_update<VAR>(H, r, ke, lane, rc.y, +1);
                                 }
                             }
                         }
@@ -367,7 +367,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     for (int r = 0; r < LP_R; ++r) {
                         if (valid[r]) {
                             int ke = exact_bin(ui, per[r], LP_ROWS);
-                            hist_update<VAR>(H, r, ke, lane, qi, +1);
+                            if (ke >= 0) hist_update<VAR>(H, r, ke, lane, qi, +1);
                         }
                     }
                 }

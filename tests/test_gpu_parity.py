@@ -132,6 +132,7 @@ def test_ragged_batch_edge_cases(gp, ref, nbins):
     periods[6] = np.inf
     periods[7] = 1e-9            # x far outside the fast range
     periods[8] = 1e9
+    periods[9] = 1e-320          # (t - t0) / P overflows: samples skipped (R20)
     t0 = np.linspace(-1.0, 2.0, w.ncurves)
     g = run_gpu(gp, w, periods, t0=t0)
     r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins, t0=t0)

@@ -427,3 +427,15 @@ def test_config0_recovers_injected_period_statistically(ref):
         stat = np.where(c > 0, s64 / np.sqrt(np.maximum(c, 1)), 0.0).min(axis=1)
     best = grid[int(np.argmin(stat))]
     assert min(abs(best - 0.5), abs(best - 1.0)) < 2e-3
+
+
+def test_overflowing_quotient_skips_the_sample(ref):
+    """R20: a positive period so small that (t - t0) / P overflows gives the sample no phase;
+    it is skipped (only t == t0, whose quotient is exactly 0, lands in bin 0)."""
+    t = np.array([0.0, 1.0, 2.0, -3.0])
+    f = np.array([1.0, 2.0, 4.0, 8.0], np.float32)
+    per = np.array([1e-320, 0.5])
+    s, c, s64 = ref.fold(t, f, per, 4)
+    assert c[0].tolist() == [1, 0, 0, 0] and s64[0].tolist() == [1.0, 0, 0, 0]
+    assert c[1].sum() == 4
+    assert ref.bin_index(t, 1e-320, 4).tolist() == [0, -1, -1, -1]
