@@ -28,6 +28,8 @@
 //   (exact: floor(phi * 256) >> k == floor(phi * (256 >> k))).
 // * Epilogue: lane l walks ITS periods' rows (conflict-free), so mean / std need no
 //   cross-lane reduction; every lane writes 32-byte sectors (8 bins) of its own rows.
+#include <mutex>
+
 #include "common.cuh"
 
 namespace gpfc {
@@ -36,7 +38,7 @@ namespace {
 
 constexpr int LP_THREADS = 768;
 constexpr int LP_WARPS = LP_THREADS / 32;
-constexpr int LP_EPI_WARPS = 16;              // sizes the statistics partials: (LP_WARPS / R) * 32 R <= 16 * 96
+constexpr int LP_EPI_WARPS = 8;               // sizes the statistics partials: (LP_WARPS / R) * 32 R <= 8 * 96
 constexpr int LP_GRAN = 64;                   // samples per staging granule
 constexpr unsigned LP_SMEM_BASE = 0x400;      // shared-window address of dynamic shared memory
 
@@ -93,18 +95,36 @@ __device__ __forceinline__ int hidx(int r, int row, int arr, int lane)
     return r * (256 * 64) + row * 64 + arr * 32 + lane;
 }
 
+// word index of the sum of (r, row, lane)
+template <int VAR>
+__device__ __forceinline__ int sum_word(int r, int row, int lane)
+{
+    if (VAR == 0) return hidx(r, row, 0, lane);
+    return row * 32 + lane;
+}
+
+// word index and half-word of the packed count of (r, row, lane), and the value that adds
+// one sample to it
+template <int VAR>
+__device__ __forceinline__ int cnt_word(int r, int row, int lane)
+{
+    return LP_CNT1_OFF / 4 + (row & 511) * 32 + lane;
+}
+template <int VAR>
+__device__ __forceinline__ unsigned cnt_unit(int r, int row)
+{
+    return 1u + ((unsigned)(row >> 9) << 16);   // low half counts both rows
+}
+
 // generic (slow-path) update of one sample: move = +1 adds it to `row`, -1 removes it
 template <int VAR>
 __device__ __forceinline__ void hist_update(unsigned *H, int r, int row, int lane, int q, int move)
 {
-    if (VAR == 0) {
-        atomicAdd(&H[hidx(r, row, 0, lane)], (unsigned)(move * q));
+    atomicAdd(&H[sum_word<VAR>(r, row, lane)], (unsigned)(move * q));
+    if (VAR == 0)
         atomicAdd(&H[hidx(r, row, 1, lane)], (unsigned)move);
-    } else {
-        atomicAdd(&H[row * 32 + lane], (unsigned)(move * q));
-        atomicAdd(&H[LP_CNT1_OFF / 4 + (row & 511) * 32 + lane],
-                  (unsigned)(move * (1 + ((row >> 9) << 16))));
-    }
+    else
+        atomicAdd(&H[cnt_word<VAR>(r, row, lane)], (unsigned)move * cnt_unit<VAR>(r, row));
 }
 
 // one bin = M consecutive rows: exact sum and count
@@ -116,19 +136,16 @@ __device__ __forceinline__ void read_bin(const unsigned *H, int r, int row0, int
     c = 0;
     for (int jj = 0; jj < M; ++jj) {
         const int row = row0 + jj;
+        S += (int)H[sum_word<VAR>(r, row, lane)];
         if (VAR == 0) {
-            const int i0 = hidx(r, row, 0, lane);
-            S += (int)H[i0];
-            c += H[i0 + 32];
+            c += H[hidx(r, row, 1, lane)];
         } else {
-            S += (int)H[row * 32 + lane];
-            const unsigned w = H[LP_CNT1_OFF / 4 + (row & 511) * 32 + lane];
+            const unsigned w = H[cnt_word<VAR>(r, row, lane)];
             c += (row >> 9) ? (w >> 16) : ((w & 0xffffu) - (w >> 16));
         }
     }
 }
 
-// one point-period of the fast path for period slot r (compile-time)
 // sq / c for a count c in [1, 2^32): reciprocal from an fp32 seed + two Newton steps
 // (relative error < 2^-49), then one residual correction.  The result is exact whenever the
 // quotient is representable (what the flat-profile test needs) and within 1 ulp otherwise.
@@ -217,7 +234,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
     const int mshift = V::ROWLOG - (31 - __clz(nb));   // rows merged per bin = 1 << mshift
     const int M = 1 << mshift;
     // 1.5 * 2^(52 + ROWLOG): ulp = LP_ROWS
-    const double M2 = (VAR == 0) ? 1729382256910270464.0 : 6917529027641081856.0;
+    const double M2 = (V::ROWLOG == 8) ? 1729382256910270464.0 : 6917529027641081856.0;
     const bool want_norm = a.out_norm != nullptr;
 
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
@@ -457,15 +474,22 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
         }
         } else {
         {
-            // packed variant, sweep 1: sums and counts out; one-pass moments.  Count words are
-            // shared by rows k and k + 512, so nothing is cleared here unless this is the only
-            // sweep (then the sums are cleared; the counts are cleared below)
+            // packed variants, sweep 1: sums and counts out; one-pass moments.  Count words are
+            // shared by two rows, so the counts are cleared
+            // after the last sweep; the sums are cleared here if this is the only sweep.
+            // Warp group g = warp / WPR takes period slot r = g.
+            constexpr int WPR = LP_WARPS / LP_R;
+            static_assert(LP_WARPS % LP_R == 0, "warps per period slot");
+            const int r = warp / WPR, wr = warp - r * WPR;
             double s1 = 0.0, s2 = 0.0;
             int kk = 0;
-            const long long j = p0 + lane;
+            const long long j = p0 + r * 32 + lane;
             const bool live = j < a.nperiods;
-            const bool ok = live && valid[0];
-            for (int oct = warp; oct < octs; oct += LP_WARPS) {
+            bool ok = false;
+#pragma unroll
+            for (int rr = 0; rr < LP_R; ++rr)
+                if (rr == r) ok = live && valid[rr];
+            for (int oct = wr; oct < octs; oct += WPR) {
                 float fs[8];
                 unsigned fc[8];
 #pragma unroll
@@ -473,9 +497,9 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     const int row0 = (oct * 8 + e) * M;
                     int S;
                     unsigned c;
-                    read_bin<VAR>(H, 0, row0, M, lane, S, c);
+                    read_bin<VAR>(H, r, row0, M, lane, S, c);
                     if (!want_norm)
-                        for (int jj = 0; jj < M; ++jj) H[(row0 + jj) * 32 + lane] = 0u;
+                        for (int jj = 0; jj < M; ++jj) H[sum_word<VAR>(r, row0 + jj, lane)] = 0u;
                     if (!ok) {
                         S = 0;
                         c = 0;
@@ -505,9 +529,9 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 }
             }
             if (want_norm) {
-                ps1[warp * LP_GROUP + lane] = s1;
-                ps2[warp * LP_GROUP + lane] = s2;
-                pkk[warp * LP_GROUP + lane] = kk;
+                ps1[wr * LP_GROUP + r * 32 + lane] = s1;
+                ps2[wr * LP_GROUP + r * 32 + lane] = s2;
+                pkk[wr * LP_GROUP + r * 32 + lane] = kk;
             }
         }
         }
@@ -570,33 +594,41 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 }
             }
             } else {
-            // packed variant, sweep 2: bin means recomputed from the exact sums and counts,
-            // normalised profile out, sums cleared
-            for (int oct = warp; oct < octs; oct += LP_WARPS) {
-                const long long j = p0 + lane;
+            // packed variants, sweep 2: bin means recomputed from the exact sums and counts,
+            // normalised profile out, sums cleared (same split as sweep 1)
+            {
+                constexpr int WPR = LP_WARPS / LP_R;
+                const int r = warp / WPR, wr = warp - r * WPR;
+                const long long j = p0 + r * 32 + lane;
                 const bool live = j < a.nperiods;
-                const double mu = st_mu[lane], isd = st_isd[lane];
-                const double base_o = (live && valid[0] && st_kk[lane] > 0) ? __dadd_rn(mu, center) : 0.0;
-                float fn[8];
+                bool okr = false;
 #pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int row0 = (oct * 8 + e) * M;
-                    int S;
-                    unsigned c;
-                    read_bin<VAR>(H, 0, row0, M, lane, S, c);
-                    for (int jj = 0; jj < M; ++jj) H[(row0 + jj) * 32 + lane] = 0u;
-                    double o = base_o;
-                    if (c > 0 && isd > 0.0) {
-                        const double m = div_by_count(__dmul_rn((double)S, inv_scale), c);
-                        o = __dadd_rn(o, __dmul_rn(__dsub_rn(m, mu), isd));
+                for (int rr = 0; rr < LP_R; ++rr)
+                    if (rr == r) okr = valid[rr];
+                const double mu = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
+                const double base_o = (live && okr && st_kk[r * 32 + lane] > 0) ? __dadd_rn(mu, center) : 0.0;
+                for (int oct = wr; oct < octs; oct += WPR) {
+                    float fn[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int row0 = (oct * 8 + e) * M;
+                        int S;
+                        unsigned c;
+                        read_bin<VAR>(H, r, row0, M, lane, S, c);
+                        for (int jj = 0; jj < M; ++jj) H[sum_word<VAR>(r, row0 + jj, lane)] = 0u;
+                        double o = base_o;
+                        if (okr && c > 0 && isd > 0.0) {
+                            const double m = div_by_count(__dmul_rn((double)S, inv_scale), c);
+                            o = __dadd_rn(o, __dmul_rn(__dsub_rn(m, mu), isd));
+                        }
+                        fn[e] = (float)o;
                     }
-                    fn[e] = (float)o;
-                }
-                if (live) {
-                    float4 *o4 = reinterpret_cast<float4 *>(
-                        a.out_norm + ((curve * a.nperiods + j) * nb) + oct * 8);
-                    o4[0] = make_float4(fn[0], fn[1], fn[2], fn[3]);
-                    o4[1] = make_float4(fn[4], fn[5], fn[6], fn[7]);
+                    if (live) {
+                        float4 *o4 = reinterpret_cast<float4 *>(
+                            a.out_norm + ((curve * a.nperiods + j) * nb) + oct * 8);
+                        o4[0] = make_float4(fn[0], fn[1], fn[2], fn[3]);
+                        o4[1] = make_float4(fn[4], fn[5], fn[6], fn[7]);
+                    }
                 }
             }
             }
@@ -604,7 +636,8 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
         if constexpr (V::PACKED) {
             // every row has been read: clear the packed counts
             __syncthreads();
-            for (int i = tid; i < 512 * 32; i += LP_THREADS) H[LP_CNT1_OFF / 4 + i] = 0u;
+            for (int i = tid; i < (LP_HIST_BYTES - LP_CNT1_OFF) / 4; i += LP_THREADS)
+                H[LP_CNT1_OFF / 4 + i] = 0u;
         }
         if (tid == 0) *ctr = 0;
         __syncthreads();   // B: H is zero again, tile counter reset
@@ -625,7 +658,9 @@ template <int VAR>
 static cudaError_t launch_lp_var(FoldArgs a, cudaStream_t st)
 {
     static int state = 0;   // 0 = not initialised, 1 = ready, -1 = shared-memory base differs
+    static std::mutex init_mutex;
     auto kern = fold_lp_kernel<VAR>;
+    std::unique_lock<std::mutex> lock(init_mutex);
     if (state == 0) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              LP_SMEM_BYTES);
@@ -640,7 +675,9 @@ static cudaError_t launch_lp_var(FoldArgs a, cudaStream_t st)
         if (e != cudaSuccess) return e;
         state = (h == LP_SMEM_BASE) ? 1 : -1;
     }
-    if (state < 0) return cudaErrorInvalidConfiguration;   // never seen; reported, not worked around
+    const int ready = state;
+    lock.unlock();
+    if (ready < 0) return cudaErrorInvalidConfiguration;   // never seen; reported, not worked around
     constexpr int GROUP = 32 * LpV<VAR>::R;
     const long long ngroups = (a.nperiods + GROUP - 1) / GROUP;
     const long long nitems = ngroups * a.ncurves;

@@ -145,10 +145,11 @@ def test_ragged_batch_edge_cases(gp, ref, nbins):
     check(g0, r0)
 
 
-@pytest.mark.parametrize("nbins", [512, 1024])
+@pytest.mark.parametrize("nbins", [64, 256, 512, 1024])
 def test_packed_counts_long_and_short_curves(gp, ref, nbins):
-    """nbins 512 / 1024 pack two rows' counts in one word (curves of up to 65,535 samples);
-    a longer curve in the same batch is folded by the generic kernel.  Cadence-locked
+    """The fast kernels pack two 16-bit counts in one word (two rows at nbins 512 / 1024, two
+    period slots at nbins <= 256), which holds for curves of up to 65,535 samples; a longer
+    curve in the same batch is folded by a second launch (unpacked / generic kernel).  Cadence-locked
     periods put thousands of samples in one bin."""
     rng = np.random.default_rng(11)
     dt = workloads.KEPLER_CADENCE_D
