@@ -36,9 +36,8 @@ namespace gpfc {
 
 namespace {
 
-constexpr int LP_THREADS = 768;
-constexpr int LP_WARPS = LP_THREADS / 32;
-constexpr int LP_EPI_WARPS = 8;               // sizes the statistics partials: (LP_WARPS / R) * 32 R <= 8 * 96
+constexpr int LP_MAX_WARPS = 24;              // largest variant: sizes the staging area
+constexpr int LP_EPI_WARPS = 8;               // sizes the statistics partials: (warps / R) * 32 R <= 8 * 96
 constexpr int LP_GRAN = 64;                   // samples per staging granule
 constexpr unsigned LP_SMEM_BASE = 0x400;      // shared-window address of dynamic shared memory
 
@@ -50,11 +49,11 @@ constexpr unsigned LP_SMEM_BASE = 0x400;      // shared-window address of dynami
 //          (nbins 512, 1024; longer curves are left to fold_generic_kernel).
 template <int VAR> struct LpV;
 template <> struct LpV<0> {
-    static constexpr int R = 3, ROWLOG = 8;
+    static constexpr int R = 3, ROWLOG = 8, THREADS = 768;
     static constexpr bool PACKED = false;
 };
 template <> struct LpV<1> {
-    static constexpr int R = 1, ROWLOG = 10;
+    static constexpr int R = 1, ROWLOG = 10, THREADS = 768;
     static constexpr bool PACKED = true;
 };
 constexpr int LP_GROUP_MAX = 96;              // periods per work item, largest variant
@@ -64,7 +63,7 @@ constexpr int LP_HIST_BYTES = 196608;         // both variants
 constexpr int LP_CNT1_OFF = 131072;           // VAR 1: byte offset of the packed counts
 // scratch after the histograms: sample staging during the fold, statistics partials in the
 // epilogue (the two never live at the same time)
-constexpr int LP_STAGE_OFF = LP_HIST_BYTES;                   // int2 [LP_WARPS][LP_GRAN]
+constexpr int LP_STAGE_OFF = LP_HIST_BYTES;                   // int2 [warps][LP_GRAN]
 constexpr int LP_PS1_OFF = LP_HIST_BYTES;                     // double [LP_EPI_WARPS][GROUP]
 constexpr int LP_PS2_OFF = LP_PS1_OFF + LP_EPI_WARPS * LP_GROUP_MAX * 8;
 constexpr int LP_PKK_OFF = LP_PS2_OFF + LP_EPI_WARPS * LP_GROUP_MAX * 8;   // int [LP_EPI_WARPS][GROUP]
@@ -75,7 +74,7 @@ constexpr int LP_CTR_OFF = LP_KK_OFF + LP_GROUP_MAX * 4;
 constexpr int LP_SMEM_BYTES = LP_CTR_OFF + 16;
 static_assert(LP_SMEM_BYTES <= 227 * 1024, "shared memory budget");
 static_assert(GPFC_TILE == 2 * LP_GRAN, "half-tile work units are one staging granule");
-static_assert(LP_WARPS * LP_GRAN * 8 <= LP_MU_OFF - LP_STAGE_OFF, "staging fits in the scratch");
+static_assert(LP_MAX_WARPS * LP_GRAN * 8 <= LP_MU_OFF - LP_STAGE_OFF, "staging fits in the scratch");
 
 // shared-memory reductions with an immediate offset: ATOMS.ADD / ATOMS.POPC.INC
 template <int IMM>
@@ -89,17 +88,18 @@ __device__ __forceinline__ void red_inc(unsigned addr)
     asm volatile("red.shared.add.u32 [%0+%1], 1;" ::"r"(addr), "n"(IMM) : "memory");
 }
 
-// word index of (r, row, array, lane) in the VAR 0 histogram
+// word index of (r, row, array, lane) in the unpacked histogram [r][row][sum|count][lane]
+template <int VAR>
 __device__ __forceinline__ int hidx(int r, int row, int arr, int lane)
 {
-    return r * (256 * 64) + row * 64 + arr * 32 + lane;
+    return r * (64 << LpV<VAR>::ROWLOG) + row * 64 + arr * 32 + lane;
 }
 
 // word index of the sum of (r, row, lane)
 template <int VAR>
 __device__ __forceinline__ int sum_word(int r, int row, int lane)
 {
-    if (VAR == 0) return hidx(r, row, 0, lane);
+    if (!LpV<VAR>::PACKED) return hidx<VAR>(r, row, 0, lane);
     return row * 32 + lane;
 }
 
@@ -121,8 +121,8 @@ template <int VAR>
 __device__ __forceinline__ void hist_update(unsigned *H, int r, int row, int lane, int q, int move)
 {
     atomicAdd(&H[sum_word<VAR>(r, row, lane)], (unsigned)(move * q));
-    if (VAR == 0)
-        atomicAdd(&H[hidx(r, row, 1, lane)], (unsigned)move);
+    if (!LpV<VAR>::PACKED)
+        atomicAdd(&H[hidx<VAR>(r, row, 1, lane)], (unsigned)move);
     else
         atomicAdd(&H[cnt_word<VAR>(r, row, lane)], (unsigned)move * cnt_unit<VAR>(r, row));
 }
@@ -137,8 +137,8 @@ __device__ __forceinline__ void read_bin(const unsigned *H, int r, int row0, int
     for (int jj = 0; jj < M; ++jj) {
         const int row = row0 + jj;
         S += (int)H[sum_word<VAR>(r, row, lane)];
-        if (VAR == 0) {
-            c += H[hidx(r, row, 1, lane)];
+        if (!LpV<VAR>::PACKED) {
+            c += H[hidx<VAR>(r, row, 1, lane)];
         } else {
             const unsigned w = H[cnt_word<VAR>(r, row, lane)];
             c += (row >> 9) ? (w >> 16) : ((w & 0xffffu) - (w >> 16));
@@ -203,11 +203,14 @@ struct ForR {
 };
 
 template <int VAR>
-__global__ void __launch_bounds__(LP_THREADS, 1)
+__global__ void __launch_bounds__(LpV<VAR>::THREADS, 1)
 fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
 {
     using V = LpV<VAR>;
     constexpr int LP_R = V::R, LP_ROWS = 1 << V::ROWLOG, LP_GROUP = 32 * V::R;
+    constexpr int LP_THREADS = V::THREADS, LP_WARPS = V::THREADS / 32;
+    static_assert(LP_WARPS <= LP_MAX_WARPS, "staging area");
+    static_assert((LP_WARPS / LP_R) * LP_GROUP <= LP_EPI_WARPS * LP_GROUP_MAX, "statistics partials");
     extern __shared__ __align__(1024) unsigned char smem[];
     if (probe) {   // report where dynamic shared memory starts (host checks LP_SMEM_BASE once)
         if (threadIdx.x == 0 && blockIdx.x == 0) *probe = (unsigned)__cvta_generic_to_shared(smem);
@@ -668,7 +671,7 @@ static cudaError_t launch_lp_var(FoldArgs a, cudaStream_t st)
         unsigned *d = nullptr, h = 0;
         e = cudaMalloc(reinterpret_cast<void **>(&d), sizeof(unsigned));
         if (e != cudaSuccess) return e;
-        kern<<<1, LP_THREADS, LP_SMEM_BYTES, st>>>(a, 0, 0, d);
+        kern<<<1, LpV<VAR>::THREADS, LP_SMEM_BYTES, st>>>(a, 0, 0, d);
         e = cudaMemcpyAsync(&h, d, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         cudaFree(d);
@@ -682,7 +685,7 @@ static cudaError_t launch_lp_var(FoldArgs a, cudaStream_t st)
     const long long ngroups = (a.nperiods + GROUP - 1) / GROUP;
     const long long nitems = ngroups * a.ncurves;
     const long long grid = nitems < num_sms() ? nitems : num_sms();
-    kern<<<(unsigned)grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems, nullptr);
+    kern<<<(unsigned)grid, LpV<VAR>::THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems, nullptr);
     return cudaGetLastError();
 }
 
