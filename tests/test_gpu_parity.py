@@ -263,3 +263,72 @@ def test_empty_and_error_paths(gp):
         gp.gpfc_fold(e64, e32, per, 5000)
     with pytest.raises(gp.GpfcError):
         gp.gpfc_fold(torch.empty(4, dtype=torch.float64), e32, per, 16)   # host tensor
+
+
+def test_host_path_streams_several_chunks(gp, ref):
+    """gpfc_fold_batch_host folds the curves in chunks of about 512 MB of output and copies
+    chunk k back while chunk k+1 is folded: 20 curves x 20,000 periods x 256 bins x 3 arrays
+    = 1.2 GB = 3 chunks.  Per-curve t0, ragged lengths; sampled rows against the oracle."""
+    rng = np.random.default_rng(21)
+    curves = []
+    for c in range(20):
+        n = int(rng.integers(2000, 6000))
+        t = np.sort(rng.uniform(0.0, 90.0, n))
+        f = (rng.integers(-3000, 3000, n).astype(np.float32)) * np.float32(2.0 ** -22)
+        curves.append((t, f, None))
+    npd = 20000
+    w = workloads._pack("host_chunks", -1, curves, 0.2, 1.0, npd, 256, False)
+    periods = ref.make_period_grid(w.pmin, w.pmax, npd, w.grid_mode)
+    t0 = np.linspace(-2.0, 2.0, w.ncurves)
+    shape = (w.ncurves, npd, 256)
+    s = np.empty(shape, np.float32)
+    c = np.empty(shape, np.uint32)
+    nrm = np.empty(shape, np.float32)
+    gp.gpfc_fold_batch_host(w.times, w.flux, w.offsets, periods, 256, t0=t0, out_sum=s,
+                            out_count=c, out_norm=nrm)
+    idx = np.array(sorted(set(rng.integers(0, npd, 25).tolist()) | {0, npd - 1}))
+    for cu in (0, 7, 8, 15, 16, 19):          # first / last curves of each chunk
+        a, b = int(w.offsets[cu]), int(w.offsets[cu + 1])
+        r = ref.fold_batch(w.times[a:b], w.flux[a:b], np.array([0, b - a], np.int64), periods[idx],
+                           256, t0=t0[cu:cu + 1])
+        check({"sum": s[cu:cu + 1, idx], "count": c[cu:cu + 1, idx], "norm": nrm[cu:cu + 1, idx]}, r,
+              exact_sums=True)
+    assert np.array_equal(c.sum(axis=2, dtype=np.int64), np.broadcast_to(
+        np.diff(w.offsets)[:, None], (w.ncurves, npd)))
+
+
+def test_flat_and_sparse_profiles_fused_normalise(gp, ref):
+    """Degenerate profiles through the fused epilogue: constant flux (every bin mean equal:
+    s = 0 -> mu everywhere, exactly as the oracle), two samples, one sample, samples in one bin."""
+    t = np.arange(5000, dtype=np.float64) * 0.0137
+    curves = [(t, np.full(5000, np.float32(3.0 * 2.0 ** -12)), None),
+              (t, np.zeros(5000, np.float32), None),
+              (np.array([0.3, 0.9]), np.array([1.0, -1.0], np.float32) * np.float32(2.0 ** -10), None),
+              (np.array([0.3]), np.array([2.0 ** -9], np.float32), None),
+              (np.full(40, 0.25) + np.arange(40) * 0.5, np.linspace(-1, 1, 40).astype(np.float32), None)]
+    periods = np.array([0.5, 0.37, 1.0, 0.25, 0.713])
+    for nbins in (32, 128, 256, 1024):
+        w = workloads._pack("flat", -1, curves, 0.2, 1.0, periods.shape[0], nbins, False)
+        g = run_gpu(gp, w, periods)
+        r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
+        check(g, r)
+        # constant-flux curves: the normalised profile is exactly flat
+        assert np.array_equal(g["norm"][0], np.full_like(g["norm"][0], np.float32(3.0 * 2.0 ** -12)))
+        assert not g["norm"][1].any()
+        gf = run_gpu(gp, w, periods, want=("norm",))
+        assert np.array_equal(gf["norm"], g["norm"])
+
+
+def test_profile_hooks_count_launches(gp):
+    w = workloads.config0(nperiods=64)
+    periods = gp.gpfc_make_period_grid(w.pmin, w.pmax, 64, w.grid_mode)
+    t, f, off = dev(w.times), dev(w.flux), dev(w.offsets)
+    gp.gpfc_fold_batch(t, f, off, periods, w.nbins)            # warm-up (one-time probe launch)
+    gp.gpfc_profile(True)
+    for _ in range(3):
+        gp.gpfc_make_period_grid(w.pmin, w.pmax, 64, w.grid_mode, out=periods)
+        gp.gpfc_fold_batch(t, f, off, periods, w.nbins)
+    p = gp.gpfc_profile_read()
+    gp.gpfc_profile(False)
+    assert p["fold_launches"] == 3 and p["kernel_launches"] == 3 * 4
+    assert 0.0 < p["fold_kernel_ms"] < 1000.0
