@@ -18,7 +18,7 @@ namespace gpfc {
 namespace {
 
 constexpr int MERGE_THREADS = 512;   // fewer when nb2 is large (8 (nb2 + 1) bytes per warp)
-constexpr int MERGE_SEG = 1024;      // fine bins staged per pass (per warp: 8.4 KB)
+constexpr int MERGE_SEG = 512;       // fine bins staged per pass (per warp: 4.3 KB)
 
 __global__ void __launch_bounds__(MERGE_THREADS)
 merge_equal_count_kernel(const float *__restrict__ sum, const uint32_t *__restrict__ count,
