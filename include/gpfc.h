@@ -191,7 +191,9 @@ int gpfc_profile_read(double *fold_kernel_ms, int64_t *fold_launches, int64_t *k
  *   [0] conflict-free shared-memory atomic lane-updates / s (ATOMS.ADD + ATOMS.POPC.INC mix)
  *   [1] fp64 (DMUL + DADD) pairs / s
  *   [2] fold inner-loop point-periods / s with conflict-free bins (issue-bound ceiling)
- *   [3..7] reserved (0)
+ *   [3] fp32 atomicAdd lane-updates / s on shared memory (a CAS loop on sm_100a), pattern of [0]
+ *   [4] plain LDS + add + STS lane-updates / s on warp-private rows (no atomics)
+ *   [5..7] reserved (0)
  * Synchronous.
  */
 int gpfc_measure_peaks(double *out);

@@ -245,7 +245,8 @@ def gpfc_measure_peaks() -> dict:
     _use_current_stream()
     _check(lib().gpfc_measure_peaks(out), "gpfc_measure_peaks")
     return {"smem_atomic_lane_updates_per_s": out[0], "fp64_mul_add_pairs_per_s": out[1],
-            "fold_loop_pp_per_s": out[2]}
+            "fold_loop_pp_per_s": out[2], "smem_cas_float_lane_updates_per_s": out[3],
+            "smem_lds_sts_lane_updates_per_s": out[4]}
 
 
 def gpfc_profile(enable: bool) -> None:

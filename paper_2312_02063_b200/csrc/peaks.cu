@@ -4,6 +4,8 @@
 //   [0] conflict-free shared-memory atomic lane-updates/s: every lane owns a bank,
 //       half ATOMS.ADD, half ATOMS.POPC.INC, addresses precomputed, no other work
 //   [1] fp64 DMUL + DADD(round-down) pairs/s
+//   [3] fp32 atomicAdd on shared memory (CAS loop), same access pattern as [0]
+//   [4] plain LDS + add + STS on warp-private rows (no atomics)
 //   [2] the fold's inner loop (DMUL, DADD.RM, bin/address, guard, 2 atomics) with
 //       lane-private columns and samples in registers: the issue-bound ceiling of
 //       the main loop, with no loads, epilogue or barriers
@@ -40,6 +42,60 @@ __global__ void __launch_bounds__(1024, 1) peak_atoms_kernel(int iters, unsigned
     __syncthreads();
     unsigned acc = 0;
     for (int i = threadIdx.x; i < ROWS * 32; i += blockDim.x) acc += h[i];
+    if (acc == 0xdeadbeefu) sink[0] = acc;
+}
+
+// [3] the same access pattern with fp32 atomicAdd (a compare-and-swap loop on sm_100a) and
+// [4] with plain LDS + IADD + STS on warp-private rows (no atomics): the two alternatives to
+// native integer atomics that the design rejected.
+__global__ void __launch_bounds__(1024, 1) peak_casf_kernel(int iters, float *sink)
+{
+    float *h = reinterpret_cast<float *>(peaks_smem);   // [rows][32]
+    constexpr int ROWS = 1024;
+    const int lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < ROWS * 32; i += blockDim.x) h[i] = 0.f;
+    __syncthreads();
+    unsigned idx[8];
+    unsigned s = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 12345u;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        s = s * 1664525u + 1013904223u;
+        idx[k] = ((s >> 8) % ROWS) * 32 + lane;
+    }
+    const float v = (float)(lane + 1);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) atomicAdd(&h[idx[k]], v);
+    }
+    __syncthreads();
+    float acc = 0.f;
+    for (int i = threadIdx.x; i < ROWS * 32; i += blockDim.x) acc += h[i];
+    if (acc == -1.f) sink[0] = acc;
+}
+
+__global__ void __launch_bounds__(1024, 1) peak_ldsts_kernel(int iters, unsigned *sink)
+{
+    unsigned *h = reinterpret_cast<unsigned *>(peaks_smem);   // [warp][rows][32]: private per warp
+    constexpr int ROWS = 32;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < 32 * ROWS * 32; i += blockDim.x) h[i] = 0;
+    __syncthreads();
+    unsigned idx[8];
+    unsigned s = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 12345u;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        s = s * 1664525u + 1013904223u;
+        idx[k] = (warp * ROWS + ((s >> 8) % ROWS)) * 32 + lane;
+    }
+    const unsigned v = lane + 1;
+    volatile unsigned *hv = h;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) hv[idx[k]] = hv[idx[k]] + v;
+    }
+    __syncthreads();
+    unsigned acc = 0;
+    for (int i = threadIdx.x; i < 32 * ROWS * 32; i += blockDim.x) acc += h[i];
     if (acc == 0xdeadbeefu) sink[0] = acc;
 }
 
@@ -119,8 +175,12 @@ cudaError_t measure_peaks(double *out, cudaStream_t st)
                          (int)smem_atoms);
     cudaFuncSetAttribute(peak_loop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          (int)smem_loop);
+    cudaFuncSetAttribute(peak_casf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)smem_atoms);
+    cudaFuncSetAttribute(peak_ldsts_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)smem_atoms);
     const int iters = 4000, nper = 4000;
-    for (int which = 0; which < 3; ++which) {
+    for (int which = 0; which < 5; ++which) {
         float best = 1e30f;
         for (int rep = 0; rep < 4; ++rep) {
             cudaEventRecord(a, st);
@@ -128,8 +188,12 @@ cudaError_t measure_peaks(double *out, cudaStream_t st)
                 peak_atoms_kernel<<<sms, 1024, smem_atoms, st>>>(iters, (unsigned *)sink);
             else if (which == 1)
                 peak_fp64_kernel<<<sms * 2, 1024, 0, st>>>(iters, 1e-3, (double *)sink);
-            else
+            else if (which == 2)
                 peak_loop_kernel<<<sms, 1024, smem_loop, st>>>(nper, 0.25, (unsigned *)sink);
+            else if (which == 3)
+                peak_casf_kernel<<<sms, 1024, smem_atoms, st>>>(iters / 4, (float *)sink);
+            else
+                peak_ldsts_kernel<<<sms, 1024, smem_atoms, st>>>(iters, (unsigned *)sink);
             cudaEventRecord(b, st);
             e = cudaEventSynchronize(b);
             if (e != cudaSuccess) break;
@@ -142,6 +206,8 @@ cudaError_t measure_peaks(double *out, cudaStream_t st)
         if (which == 0) units = (double)sms * 1024 * iters * 8.0;
         if (which == 1) units = (double)sms * 2 * 1024 * iters * 8.0;
         if (which == 2) units = (double)sms * 1024 * nper * 4.0;
+        if (which == 3) units = (double)sms * 1024 * (iters / 4) * 8.0;
+        if (which == 4) units = (double)sms * 1024 * iters * 8.0;
         out[which] = units / (best * 1e-3);
     }
     cudaEventDestroy(a);
