@@ -416,6 +416,7 @@ def gpu_arm(args):
         roof["measured_peak"] = peaks["smem_atomic_lane_updates_per_s"] / 1e9
         roof["frac_of_measured"] = achieved / peaks["smem_atomic_lane_updates_per_s"]
         roof["fp64_pairs_per_s"] = peaks["fp64_mul_add_pairs_per_s"]
+        roof["inner_loop_ceiling_pp_per_s"] = peaks["fold_loop_pp_per_s"]   # fold_lp<0> loop alone
         roof["alternatives_lane_updates_per_s"] = {
             "cas_float_atomicAdd": peaks["smem_cas_float_lane_updates_per_s"],
             "lds_add_sts_private_rows": peaks["smem_lds_sts_lane_updates_per_s"]}

@@ -190,7 +190,8 @@ int gpfc_profile_read(double *fold_kernel_ms, int64_t *fold_launches, int64_t *k
  * and clocks.  out (host, double[8]):
  *   [0] conflict-free shared-memory atomic lane-updates / s (ATOMS.ADD + ATOMS.POPC.INC mix)
  *   [1] fp64 (DMUL + DADD) pairs / s
- *   [2] fold inner-loop point-periods / s with conflict-free bins (issue-bound ceiling)
+ *   [2] point-periods / s of the fold kernel's inner loop alone (no global loads, tile set-up,
+ *       epilogue or barriers): the ceiling of the kernel design
  *   [3] fp32 atomicAdd lane-updates / s on shared memory (a CAS loop on sm_100a), pattern of [0]
  *   [4] plain LDS + add + STS lane-updates / s on warp-private rows (no atomics)
  *   [5..7] reserved (0)

@@ -6,9 +6,9 @@
 //   [1] fp64 DMUL + DADD(round-down) pairs/s
 //   [3] fp32 atomicAdd on shared memory (CAS loop), same access pattern as [0]
 //   [4] plain LDS + add + STS on warp-private rows (no atomics)
-//   [2] the fold's inner loop (DMUL, DADD.RM, bin/address, guard, 2 atomics) with
-//       lane-private columns and samples in registers: the issue-bound ceiling of
-//       the main loop, with no loads, epilogue or barriers
+//   [2] the inner loop of fold_lp_kernel<0> alone (DFMA.RM, PRMT, VIMNMX3, 2 atomics per
+//       point-period, samples broadcast from shared memory): the ceiling of the fold loop
+//       with no global loads, tile set-up, epilogue or barriers
 #include "common.cuh"
 
 namespace gpfc {
@@ -119,40 +119,61 @@ __global__ void __launch_bounds__(1024, 1) peak_fp64_kernel(int iters, double se
     if (acc == 0xdeadbeefu) sink[0] = (double)acc;
 }
 
-__global__ void __launch_bounds__(1024, 1) peak_loop_kernel(int nper, double seed, unsigned *sink)
+// [2] the inner loop of fold_lp_kernel<0> alone (lane = period, 3 periods per lane, 8-byte
+// sample records broadcast from shared memory, DFMA.RM + PRMT + VIMNMX3 + ATOMS.ADD +
+// ATOMS.POPC.INC per point-period): no global loads, tile set-up, epilogue or barriers.
+template <int IMM>
+__device__ __forceinline__ void pk_red_add(unsigned addr, int v)
 {
-    constexpr int NBLOG = 8, NB = 256, KS = 4;
-    int *H = reinterpret_cast<int *>(peaks_smem);   // [2][NB][32]
-    const int lane = threadIdx.x & 31;
-    for (int i = threadIdx.x; i < 2 * NB * 32; i += blockDim.x) H[i] = 0;
+    asm volatile("red.shared.add.u32 [%0+%2], %1;" ::"r"(addr), "r"(v), "n"(IMM) : "memory");
+}
+template <int IMM>
+__device__ __forceinline__ void pk_red_inc(unsigned addr)
+{
+    asm volatile("red.shared.add.u32 [%0+%1], 1;" ::"r"(addr), "n"(IMM) : "memory");
+}
+
+__global__ void __launch_bounds__(768, 1) peak_loop_kernel(int nsamples, double seed, unsigned *sink)
+{
+    unsigned *H = reinterpret_cast<unsigned *>(peaks_smem);          // [3][256][2][32]
+    int4 *rec = reinterpret_cast<int4 *>(peaks_smem + 196608);        // 64 records of 8 bytes x 2
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < 49152; i += blockDim.x) H[i] = 0;
+    if (threadIdx.x < 64)
+        rec[threadIdx.x] = make_int4(threadIdx.x * 40503 + 17, (int)threadIdx.x - 30,
+                                     threadIdx.x * 65599 + 3, 31 - (int)threadIdx.x);
     __syncthreads();
-    double u[KS];
-    int q[KS];
+    const unsigned lane4 = (unsigned)lane << 2;   // + 0x400 (shared-window base) in the immediates
+    double rp[3], C[3];
 #pragma unroll
-    for (int k = 0; k < KS; ++k) {
-        u[k] = 0.020433 * (double)(blockIdx.x * 4096 + k * 1024 + threadIdx.x) + seed;
-        q[k] = (int)threadIdx.x - 500 + k;
+    for (int r = 0; r < 3; ++r) {
+        rp[r] = (256.0 + 8.0 * (r * 32 + lane)) * 0.020433 * (1.0 / 33554432.0) * (1.0 + seed);
+        C[r] = 1048576.0 + (double)((r * 97 + lane * 13) & 255) + 0.375;
     }
-    const double MAGIC = 6755399441055744.0 / (double)(1ull << (32 - NBLOG));
     unsigned gmin = 0xffffffffu;
-    double r = 256.0;
-    for (int p = 0; p < nper; ++p) {
+    for (int s0 = warp * 4; s0 < nsamples; s0 += 4 * (blockDim.x >> 5)) {
+        const int4 ra = rec[(s0 >> 1) & 31], rb = rec[((s0 >> 1) + 1) & 31];
+        const unsigned iv[4] = {(unsigned)ra.x + s0, (unsigned)ra.z + s0, (unsigned)rb.x + s0,
+                                (unsigned)rb.z + s0};
+        const int q[4] = {ra.y, ra.w, rb.y, rb.w};
 #pragma unroll
-        for (int k = 0; k < KS; ++k) {
-            double y = __dmul_rn(u[k], r);
-            double mm = __dadd_rd(y, MAGIC);
-            unsigned lo = (unsigned)__double2loint(mm);
-            unsigned bin = lo >> (32 - NBLOG);
-            gmin = min(gmin, lo * (unsigned)NB + (unsigned)NB);
-            int *hs = H + bin * 32 + lane;
-            atomicAdd(hs, q[k]);
-            atomicAdd(reinterpret_cast<unsigned *>(hs + NB * 32), 1u);
+        for (int k = 0; k < 4; ++k) {
+            const double v = (double)iv[k];
+#pragma unroll
+            for (int r = 0; r < 3; ++r) {
+                double m = __fma_rd(v, rp[r], C[r]);
+                unsigned lo = (unsigned)__double2loint(m), hi = (unsigned)__double2hiint(m);
+                unsigned addr = __byte_perm(lane4, hi, 0x3240);
+                gmin = min(gmin, lo);
+                if (r == 0) { pk_red_add<0x400>(addr, q[k]); pk_red_inc<0x400 + 128>(addr); }
+                if (r == 1) { pk_red_add<0x400 + 65536>(addr, q[k]); pk_red_inc<0x400 + 65536 + 128>(addr); }
+                if (r == 2) { pk_red_add<0x400 + 131072>(addr, q[k]); pk_red_inc<0x400 + 131072 + 128>(addr); }
+            }
         }
-        r += 0.00048828125;
     }
     __syncthreads();
     unsigned acc = gmin;
-    for (int i = threadIdx.x; i < 2 * NB * 32; i += blockDim.x) acc += (unsigned)H[i];
+    for (int i = threadIdx.x; i < 49152; i += blockDim.x) acc += H[i];
     if (acc == 0xdeadbeefu) sink[0] = acc;
 }
 
@@ -170,7 +191,7 @@ cudaError_t measure_peaks(double *out, cudaStream_t st)
     cudaEvent_t a, b;
     cudaEventCreate(&a);
     cudaEventCreate(&b);
-    const size_t smem_atoms = 1024 * 32 * 4, smem_loop = 2 * 256 * 32 * 4;
+    const size_t smem_atoms = 1024 * 32 * 4, smem_loop = 196608 + 1024;
     cudaFuncSetAttribute(peak_atoms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          (int)smem_atoms);
     cudaFuncSetAttribute(peak_loop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -179,7 +200,7 @@ cudaError_t measure_peaks(double *out, cudaStream_t st)
                          (int)smem_atoms);
     cudaFuncSetAttribute(peak_ldsts_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          (int)smem_atoms);
-    const int iters = 4000, nper = 4000;
+    const int iters = 4000, nper = 400000;   // nper: samples per CTA of the loop kernel
     for (int which = 0; which < 5; ++which) {
         float best = 1e30f;
         for (int rep = 0; rep < 4; ++rep) {
@@ -189,7 +210,7 @@ cudaError_t measure_peaks(double *out, cudaStream_t st)
             else if (which == 1)
                 peak_fp64_kernel<<<sms * 2, 1024, 0, st>>>(iters, 1e-3, (double *)sink);
             else if (which == 2)
-                peak_loop_kernel<<<sms, 1024, smem_loop, st>>>(nper, 0.25, (unsigned *)sink);
+                peak_loop_kernel<<<sms, 768, smem_loop, st>>>(nper, 0.25, (unsigned *)sink);
             else if (which == 3)
                 peak_casf_kernel<<<sms, 1024, smem_atoms, st>>>(iters / 4, (float *)sink);
             else
@@ -205,7 +226,7 @@ cudaError_t measure_peaks(double *out, cudaStream_t st)
         double units = 0;
         if (which == 0) units = (double)sms * 1024 * iters * 8.0;
         if (which == 1) units = (double)sms * 2 * 1024 * iters * 8.0;
-        if (which == 2) units = (double)sms * 1024 * nper * 4.0;
+        if (which == 2) units = (double)sms * (double)nper * 96.0;
         if (which == 3) units = (double)sms * 1024 * (iters / 4) * 8.0;
         if (which == 4) units = (double)sms * 1024 * iters * 8.0;
         out[which] = units / (best * 1e-3);
