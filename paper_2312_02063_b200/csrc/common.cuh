@@ -12,7 +12,7 @@ namespace gpfc {
 // Samples are handled in anchor tiles of GPFC_TILE consecutive (compacted) samples of a
 // curve: the prepass stores, per tile, the smallest u (the anchor a) and a power-of-two
 // scale 2^-S with (max u - a) * 2^S < 2^32, and per sample the 8-byte record
-// {iv = rint((u - a) * 2^S) (uint32), q (int32)}: |iv * 2^-S - (u - a)| <= 2^-S.
+// {iv = rint((u - a) * 2^S) (uint32), q (int32)}: |iv * 2^-S - (u - a)| <= 2^-(S+1).
 constexpr int GPFC_TILE = 128;
 
 struct TileInfo {

@@ -265,7 +265,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
 
         // guard band, in units of 2^-32 row.  Per item:
         //   ebase = 4 * 2^-53 * max|u| * rpmax * 2^32 + 1     (roundings of u/P, 1/P, v, C)
-        // per tile, the quantisation of v adds  eq = 2^-S * rpmax * 2^32;
+        // per tile, the quantisation of v adds  eq = 2^-(S+1) * rpmax * 2^32;
         //   delta >= E + 1 unit, D = 2 delta  ->  D >= 2 (ebase + eq) + 2
         const double U = fmax(fabs(cm.umin), fabs(cm.umax));
         const double ebase = 4.0 * U * rpmax * (1.0 / 2097152.0) + 1.0;
@@ -290,11 +290,11 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 const int cnt = min((u < nfull) ? GPFC_TILE : LP_GRAN, n - base);
                 if (cnt <= 0) continue;
                 const TileInfo ti = a.tiles[cm.tile0 + t];
-                // D = smallest power of two >= need (>= 16): exponent trick, need = f 2^e, f < 1
-                const double need = 2.0 * (ebase + ti.inv_scale * rpmax * 4294967296.0) + 2.0;
-                int ex = ((__double2hiint(need) >> 20) & 0x7ff) - 1022;
-                if (ex < 4) ex = 4;
-                const unsigned D = 1u << ex;
+                // D = smallest even integer >= need (>= 16); the quantisation of v is a rounding
+                // to nearest: |iv 2^-S - v| <= 2^-(S+1)
+                const double need = 2.0 * (ebase + 0.5 * ti.inv_scale * rpmax * 4294967296.0) + 2.0;
+                unsigned D = ((unsigned)need + 2u) & ~1u;
+                if (D < 16u) D = 16u;
                 const double K = 1048576.0 + (double)(D >> 1) * (1.0 / 4294967296.0);
                 double C[LP_R], rps[LP_R];
 #pragma unroll

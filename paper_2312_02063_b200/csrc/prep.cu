@@ -186,6 +186,7 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
         int S = 32 - e;                        // span * 2^S < 2^32
         if (S > 40) S = 40;
         if (S < -900) S = -900;
+        if (span * ldexp(1.0, S) > 4294967294.0) S -= 1;   // rint() below never reaches 2^32
         const double scale = ldexp(1.0, S);
 #pragma unroll
         for (int k = 0; k < GPFC_TILE / 32; ++k) {
