@@ -134,6 +134,7 @@ __device__ __forceinline__ void read_bin(const unsigned *H, int r, int row0, int
 {
     S = 0;
     c = 0;
+#pragma unroll 1
     for (int jj = 0; jj < M; ++jj) {
         const int row = row0 + jj;
         S += (int)H[sum_word<VAR>(r, row, lane)];
@@ -501,8 +502,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     int S;
                     unsigned c;
                     read_bin<VAR>(H, r, row0, M, lane, S, c);
-                    if (!want_norm)
-                        for (int jj = 0; jj < M; ++jj) H[sum_word<VAR>(r, row0 + jj, lane)] = 0u;
+                    for (int jj = 0; jj < M; ++jj) H[sum_word<VAR>(r, row0 + jj, lane)] = 0u;
                     if (!ok) {
                         S = 0;
                         c = 0;
@@ -510,11 +510,18 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     const double sq = __dmul_rn((double)S, inv_scale);
                     fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
                     fc[e] = c;
-                    if (want_norm && c > 0) {
-                        const double d = __dsub_rn(div_by_count(sq, c), pivot);
-                        s1 += d;
-                        s2 += __dmul_rn(d, d);
-                        kk += 1;
+                    if (want_norm) {
+                        // deviation of the bin mean from the curve mean, kept as fp32 in the
+                        // bin's (cleared) sum word for sweep 2: NaN = empty bin
+                        float df = __int_as_float(0x7fc00000);
+                        if (c > 0) {
+                            const double d = __dsub_rn(div_by_count(sq, c), pivot);
+                            s1 += d;
+                            s2 += __dmul_rn(d, d);
+                            kk += 1;
+                            df = (float)d;
+                        }
+                        H[sum_word<VAR>(r, row0, lane)] = __float_as_uint(df);
                     }
                 }
                 if (live) {
@@ -597,8 +604,9 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 }
             }
             } else {
-            // packed variants, sweep 2: bin means recomputed from the exact sums and counts,
-            // normalised profile out, sums cleared (same split as sweep 1)
+            // packed variants, sweep 2: normalised profile from the fp32 deviations sweep 1
+            // left in the sum words (|d| is a few profile sigmas, so fp32 keeps (d - dm) / s to
+            // ~1e-6), sum words cleared (same split as sweep 1)
             {
                 constexpr int WPR = LP_WARPS / LP_R;
                 const int r = warp / WPR, wr = warp - r * WPR;
@@ -609,21 +617,18 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 for (int rr = 0; rr < LP_R; ++rr)
                     if (rr == r) okr = valid[rr];
                 const double mu = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
+                const double dm = __dsub_rn(mu, pivot);
                 const double base_o = (live && okr && st_kk[r * 32 + lane] > 0) ? __dadd_rn(mu, center) : 0.0;
                 for (int oct = wr; oct < octs; oct += WPR) {
                     float fn[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
-                        const int row0 = (oct * 8 + e) * M;
-                        int S;
-                        unsigned c;
-                        read_bin<VAR>(H, r, row0, M, lane, S, c);
-                        for (int jj = 0; jj < M; ++jj) H[sum_word<VAR>(r, row0 + jj, lane)] = 0u;
+                        const int i0 = sum_word<VAR>(r, (oct * 8 + e) * M, lane);
+                        const float df = __uint_as_float(H[i0]);
+                        H[i0] = 0u;
                         double o = base_o;
-                        if (okr && c > 0 && isd > 0.0) {
-                            const double m = div_by_count(__dmul_rn((double)S, inv_scale), c);
-                            o = __dadd_rn(o, __dmul_rn(__dsub_rn(m, mu), isd));
-                        }
+                        if (okr && df == df && isd > 0.0)
+                            o = __dadd_rn(o, __dmul_rn(__dsub_rn((double)df, dm), isd));
                         fn[e] = (float)o;
                     }
                     if (live) {
@@ -691,11 +696,17 @@ static cudaError_t launch_lp_var(FoldArgs a, cudaStream_t st)
 
 cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st)
 {
-    if (a.nbins <= 256) return launch_lp_var<0>(a, st);
+    // cudaErrorInvalidConfiguration from launch_lp_var = the shared-memory window does not start
+    // where the kernels' immediates assume (never seen): the exact generic kernel takes over
+    if (a.nbins <= 256) {
+        cudaError_t e = launch_lp_var<0>(a, st);
+        return (e == cudaErrorInvalidConfiguration) ? launch_fold_generic(a, st) : e;
+    }
     // packed counts: curves of up to 65,535 valid samples here, longer ones in the generic kernel
     FoldArgs b = a;
     b.n_max = LP_PACKED_MAX_N;
     cudaError_t e = launch_lp_var<1>(b, st);
+    if (e == cudaErrorInvalidConfiguration) return launch_fold_generic(a, st);
     if (e != cudaSuccess) return e;
     b = a;
     b.n_min = LP_PACKED_MAX_N + 1;
