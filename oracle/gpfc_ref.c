@@ -34,10 +34,15 @@
  * permutation invariance, nb -> nb/2 pair merge), collapse closed forms, the
  * noiseless-box closed form, sqrt(N) noise attenuation, and
  * mean/std invariants plus a numpy cross-check for the normalisation.
- * gpfc_ref_two_tier_merge (NEXT row, not on the graded path): pinned by
- * count/sum conservation, the exact equal-count property and the
- * sort-based fold on tie-free inputs; the pro-rata split of a boundary bin is
- * a reading (R18) -- "parity unpinned" for the split values themselves.
+ * gpfc_ref_two_tier_merge ("Fourthly"): pinned by hand-worked
+ * merges with a fractional number of points per output bin, fine bins cut by
+ * one and by three boundaries and empty fine bins (tests/golden/
+ * hand_vectors.json "two_tier_merge"), the paper's own 65,536 / 256 = 256
+ * points per bin, an independent piecewise-linear
+ * interpolation of the cumulative flux in cumulative count, count/sum
+ * conservation and the sort-based fold on tie-free inputs.  The pro-rata split
+ * of a boundary bin is reading R18 (the paper does not say how a split bin's
+ * flux is shared).
  *
  * Build: gcc -O2 -std=c11 -ffp-contract=off -fno-fast-math -shared -fPIC
  * (no FMA contraction, so every operation below rounds once, as written).
@@ -360,7 +365,7 @@ int gpfc_ref_fold_batch(const double *times, const float *flux,
 }
 
 /*
- * NEXT row (not on the graded path): step 4 of PAPER.md:111 --
+ * Step 4 of PAPER.md:111 --
  * "scan the [fine] bins from left to right, combine the adjacent bins, and
  * split bins on the boundary as needed, to generate a final layout of [nb2]
  * bins ... each ... containing the same number of flux data points".

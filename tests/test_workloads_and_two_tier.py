@@ -48,9 +48,52 @@ def test_ragged_batch_has_edge_cases():
 
 # ------------------------------------------------------------------ two-tier merge (NEXT)
 
-def test_two_tier_conservation_and_equal_count(ref):
+def _interp_merge(s64, c, nb2):
+    """R18 in a different formulation from the oracle's left-to-right scan: the cumulative flux
+    is piecewise linear in cumulative count (knots after every non-empty fine bin); output bin b
+    is the difference of that function at b N/nb2 and (b + 1) N/nb2."""
+    ne = c > 0
+    xc = np.concatenate([[0.0], np.cumsum(c[ne].astype(np.float64))])
+    xs = np.concatenate([[0.0], np.cumsum(s64[ne])])
+    n = xc[-1]
+    edges = np.arange(nb2 + 1, dtype=np.float64) * (n / nb2)
+    edges[-1] = n
+    return np.diff(np.interp(edges, xc, xs))
+
+
+def test_two_tier_hand_vectors_fractional_split(ref):
+    """tests/golden/hand_vectors.json 'two_tier_merge': N/nb2 is fractional, fine bins are cut
+    by one and by three boundaries, empty fine bins sit between populated ones.  An oracle that
+    rounded its targets to whole points, split by bin width instead of by count, or scanned
+    right to left fails these."""
+    import json
+    import os
+    g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "hand_vectors.json")))
+    for case in g["two_tier_merge"]["cases"]:
+        osum, omean = ref.two_tier_merge(np.array([case["sum"]], np.float64),
+                                         np.array([case["count"]], np.uint32), case["nb2"])
+        assert list(osum[0]) == case["out_sum"], case["_work"]
+        assert list(omean[0]) == case["out_mean"], case["_work"]
+
+
+def test_two_tier_paper_example_256_points_per_bin(ref):
+    """'given a light curve comprising 65,536 data points, each of the 256 bins
+    will accommodate 65536/256 = 256 data points'.  Folding unit flux makes out_sum[b] the
+    number of points of output bin b: exactly 256 everywhere, whatever the period."""
+    n = 65536
+    t = np.arange(n, dtype=np.float64) * 0.0204          # PAPER.md:204
+    f = np.ones(n, np.float32)
+    periods = [0.2, 0.6852, 1.0, 12 * 0.0204]            # the last: cadence-commensurate, sparse
+    _, c, s64 = ref.fold(t, f, periods, 4096)
+    assert (c[3] == 0).sum() > 4000                      # nearly all fine bins empty there
+    osum, omean = ref.two_tier_merge(s64, c, 256)
+    assert np.allclose(osum, 256.0, rtol=0, atol=1e-9)
+    assert np.allclose(omean, 1.0, rtol=0, atol=1e-12)
+
+
+def test_two_tier_conservation_and_interp_formulation(ref):
     rng = np.random.default_rng(0)
-    n = 5000
+    n = 5000                                             # 5000 / 256 is fractional
     t = np.sort(rng.uniform(0, 300, n))
     f = rng.normal(0, 1e-3, n).astype(np.float32)
     periods = [0.2, 0.37, 0.99]
@@ -58,7 +101,17 @@ def test_two_tier_conservation_and_equal_count(ref):
     osum, omean = ref.two_tier_merge(s64, c, 256)
     assert osum.shape == (3, 256)
     assert np.allclose(osum.sum(axis=1), s64.sum(axis=1), rtol=0, atol=1e-12)
-    assert np.allclose(omean * (n / 256), osum, rtol=1e-12, atol=0)
+    for j in range(3):
+        want = _interp_merge(s64[j], c[j], 256)
+        assert np.allclose(osum[j], want, rtol=0, atol=1e-15 + 1e-12 * np.abs(want).max())
+        assert np.allclose(omean[j], want / (n / 256), rtol=0, atol=1e-14)
+    # ragged bin counts, nb1 not a multiple of nb2, more output than input bins
+    for nb1, nb2 in [(37, 5), (8, 12), (100, 7)]:
+        cc = rng.integers(0, 9, nb1).astype(np.uint32)
+        cc[rng.integers(0, nb1, nb1 // 3)] = 0
+        ss = rng.normal(0, 1, nb1) * (cc > 0)
+        osum, _ = ref.two_tier_merge(ss[None, :], cc[None, :], nb2)
+        assert np.allclose(osum[0], _interp_merge(ss, cc, nb2), rtol=0, atol=1e-12)
 
 
 def test_two_tier_exact_when_counts_divide(ref):
