@@ -57,6 +57,8 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-peaks", action="store_true", help="skip gpfc_measure_peaks")
+    ap.add_argument("--no-others", action="store_true",
+                    help="skip the other_configs block of the default run (configs 1, 3, 4, 5)")
     return ap.parse_args()
 
 
@@ -89,9 +91,11 @@ def workload_desc(w, args):
     if w.config_id == 5:
         return {"workload": "PAPER.md Table 1 fold: %s" % w.name, "curves": 1,
                 "samples_per_curve": int(w.n_total), "nperiods": int(w.nperiods),
-                "nbins": "4096 intermediary -> 256 equal-count", "outputs": "mean+norm [Np][256]",
+                "nbins": "4096 intermediary -> 256 equal-count (gpfc_fold_two_tier)",
+                "outputs": "mean+norm [Np][256]",
                 "grid": "uniform in period, %.1f..%.1f d" % (w.pmin, w.pmax),
-                "l2": "3.3 GB of intermediary sums + counts per step exceed the 126 MB L2"}
+                "l2": "205 MB of outputs per step exceed the 126 MB L2; the 0.84 MB curve is L2-resident "
+                      "by design (re-read by every work item)"}
     d = {"workload": "BASELINE.json configs[%d] %s" % (w.config_id, w.name),
          "curves": w.ncurves, "samples_per_curve": int(w.n_total // max(w.ncurves, 1)),
          "nperiods": int(w.nperiods), "nbins": int(w.nbins),
@@ -247,6 +251,175 @@ def reference_arm(args):
 
 
 # --------------------------------------------------------------------------- GPU arm
+def csrc_digest():
+    """sha256 over the CUDA sources: stamps the ncu captures under profiles/ (no .git on the box)."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2312_02063_b200", "csrc")
+    for f in sorted(glob.glob(os.path.join(d, "*.cu")) + glob.glob(os.path.join(d, "*.cuh"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def fold_kernel_name(w):
+    if w.nbins <= 256:
+        return "fold_lp_kernel"
+    return "fold_pk_kernel<%d>" % {512: 10, 1024: 10, 2048: 11, 4096: 12}[w.nbins]
+
+
+class DeviceRun:
+    """One workload resident in HBM: buffers, the step, its timing (CUDA events, max over ranks)."""
+
+    def __init__(self, gp, torch, w):
+        self.gp, self.torch, self.w = gp, torch, w
+        dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+        self.times, self.flux, self.offsets = dev(w.times), dev(w.flux), dev(w.offsets)
+        self.two_tier = (w.config_id == 5)
+        self.shape = (w.ncurves, w.nperiods, 256 if self.two_tier else w.nbins)
+        self.periods = torch.empty(w.nperiods, dtype=torch.float64, device="cuda")
+        f32 = lambda: torch.empty(self.shape, dtype=torch.float32, device="cuda")
+        self.out_sum = self.out_count = self.out_norm = self.out_mean = None
+        if self.two_tier:
+            self.out_mean, self.out_norm = f32(), f32()
+        else:
+            self.out_norm = f32()
+            if not w.fused_normalize:
+                self.out_sum = f32()
+                self.out_count = torch.empty(self.shape, dtype=torch.int32, device="cuda")
+        self.ws = torch.empty(gp.gpfc_workspace_bytes(w.ncurves, w.n_total, w.nperiods, w.nbins),
+                              dtype=torch.uint8, device="cuda")
+        self.noutputs = 2 if self.two_tier else (1 if w.fused_normalize else 3)
+        self.out_bytes = float(np.prod(self.shape)) * 4 * self.noutputs
+
+    def step(self):
+        gp, w = self.gp, self.w
+        gp.gpfc_make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode, out=self.periods)
+        if self.two_tier:
+            gp.gpfc_fold_two_tier(self.times, self.flux, self.offsets, self.periods, w.nbins, 256,
+                                  out_mean=self.out_mean, out_norm=self.out_norm)
+        else:
+            gp.gpfc_fold_batch(self.times, self.flux, self.offsets, self.periods, w.nbins,
+                               out_sum=self.out_sum, out_count=self.out_count, out_norm=self.out_norm)
+
+    def timed(self, steps, warmup, barrier, world, sampler=None):
+        gp, torch = self.gp, self.torch
+        gp.gpfc_set_workspace(self.ws)
+        for _ in range(warmup):
+            self.step()
+        barrier()
+        if sampler:
+            sampler.start()
+        gp.gpfc_profile(True)
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            self.step()
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        prof = gp.gpfc_profile_read()
+        paths = gp.gpfc_path_counters()
+        gp.gpfc_profile(False)
+        clocks = sampler.stop() if sampler else None
+        gp.gpfc_set_workspace(None)
+        ms = max_over_ranks(ms, world, "cuda")
+        return ms, prof, paths, clocks
+
+    def free(self):
+        for k in ("times", "flux", "offsets", "periods", "out_sum", "out_count", "out_norm",
+                  "out_mean", "ws"):
+            setattr(self, k, None)
+        self.torch.cuda.empty_cache()
+
+
+def roofline_of(w, run, prof, sm_max, peaks, traffic_db, digest):
+    """the fold kernel against the shared-memory atomic bound (2 lane-updates per
+    point-period) and, beside it, the HBM bound on its algorithmic bytes."""
+    fold_ms = prof["fold_kernel_ms"] / max(prof["fold_launches"], 1)
+    updates = 2.0 * float(w.point_periods)
+    peak_nominal = 148 * 32 * sm_max * 1e6              # 32 shared-memory atomic lanes / clk / SM
+    achieved = updates / (fold_ms * 1e-3)
+    alg_bytes = run.out_bytes + w.n_total * 12.0
+    roof = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_nominal / 1e9,
+            "unit": "G shared-atomic lane-updates/s", "frac": achieved / peak_nominal,
+            "traffic": None, "kernel": fold_kernel_name(w), "kernel_ms": fold_ms,
+            "peak_source": "derived: 148 SMs x 32 lanes/clk x %.0f MHz" % sm_max,
+            "algorithmic_bytes": alg_bytes,
+            "hbm_bound": {"algorithmic_bytes": alg_bytes,
+                          "achieved_gbs": alg_bytes / (fold_ms * 1e-3) / 1e9}}
+    try:
+        mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        roof["hbm_bound"]["peak_gbs"] = mp["hbm_gbs"]
+        roof["hbm_bound"]["peak_source"] = "MEASURED_PEAKS.json"
+    except (OSError, KeyError, ValueError):
+        roof["hbm_bound"]["peak_gbs"] = 6650.0
+        roof["hbm_bound"]["peak_source"] = "fallback (B200_PROFILING.md)"
+    roof["hbm_bound"]["frac"] = roof["hbm_bound"]["achieved_gbs"] / roof["hbm_bound"]["peak_gbs"]
+    tj = (traffic_db or {}).get(w.name)
+    if tj and (tj["curves"], tj["nperiods"], tj["nbins"]) == (w.ncurves, w.nperiods, w.nbins):
+        # DRAM bytes per launch from the committed ncu --set full capture of this workload
+        roof["traffic"] = tj["traffic_bytes"]
+        roof["traffic_source"] = "profiles/r2_traffic.json (ncu --set full of this command, sources %s)" \
+                                 % tj.get("csrc_digest", "?")
+        roof["traffic_stale"] = tj.get("csrc_digest") != digest
+    if peaks:
+        roof["measured_peak"] = peaks["smem_atomic_lane_updates_per_s"] / 1e9
+        roof["frac_of_measured"] = achieved / peaks["smem_atomic_lane_updates_per_s"]
+    return roof
+
+
+def host_e2e(gp, torch, w, run_shape, steps, barrier, world, two_tier):
+    """The same step through the host-buffer entry points: pinned host memory in and out,
+    copies inside the timed region."""
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_t, h_f, h_o = pin(w.times), pin(w.flux), pin(w.offsets)
+    h_sum = h_cnt = h_norm = None
+    if two_tier:
+        h_mean = torch.empty(run_shape, dtype=torch.float32, pin_memory=True)
+        h_norm = torch.empty(run_shape, dtype=torch.float32, pin_memory=True)
+    else:
+        h_norm = torch.empty(run_shape, dtype=torch.float32, pin_memory=True)
+        if not w.fused_normalize:
+            h_sum = torch.empty(run_shape, dtype=torch.float32, pin_memory=True)
+            h_cnt = torch.empty(run_shape, dtype=torch.int32, pin_memory=True)
+
+    def step_host():
+        if two_tier:
+            # no host entry point for the two-tier path: the user's calls are the device API
+            # with torch copies (pinned host -> device, merged profiles -> pinned host)
+            dt_, df_, do_ = (h_t.cuda(non_blocking=True), h_f.cuda(non_blocking=True),
+                             h_o.cuda(non_blocking=True))
+            per = gp.gpfc_make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode)
+            m_, n_ = gp.gpfc_fold_two_tier(dt_, df_, do_, per, w.nbins, 256)
+            h_mean.copy_(m_, non_blocking=True)
+            h_norm.copy_(n_, non_blocking=True)
+            torch.cuda.synchronize()
+            return
+        per = gp.gpfc_make_period_grid_host(w.pmin, w.pmax, w.nperiods, w.grid_mode)
+        gp.gpfc_fold_batch_host(h_t, h_f, h_o, per, w.nbins, out_sum=h_sum, out_count=h_cnt,
+                                out_norm=h_norm)
+
+    step_host()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        step_host()
+    barrier()
+    dt = max_over_ranks(time.perf_counter() - t0, world, "cuda")
+    nout = int(np.prod(run_shape)) * 4
+    e2e = {"value": float(w.point_periods) * world * steps / dt, "unit": UNIT,
+           "h2d_bytes_per_step": int(w.n_total * 12 + w.offsets.nbytes),
+           "d2h_bytes_per_step": int(nout * (1 if w.fused_normalize else 3) + w.nperiods * 8),
+           "steps": steps, "api": "gpfc_make_period_grid_host + gpfc_fold_batch_host"}
+    if two_tier:
+        e2e["d2h_bytes_per_step"] = int(2 * nout)
+        e2e["api"] = "torch H2D + gpfc_make_period_grid + gpfc_fold_two_tier + torch D2H"
+    return e2e
+
+
 def gpu_arm(args):
     import torch
     import torch.distributed as dist
@@ -261,33 +434,7 @@ def gpu_arm(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     gp.lib()
-
-    w = make_workload(args, rank)
-    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    times, flux, offsets = dev(w.times), dev(w.flux), dev(w.offsets)
-    shape = (w.ncurves, w.nperiods, w.nbins)
-    periods = torch.empty(w.nperiods, dtype=torch.float64, device="cuda")
-    two_tier = (w.config_id == 5)
-    out_norm = None if two_tier else torch.empty(shape, dtype=torch.float32, device="cuda")
-    out_sum = out_count = None
-    if two_tier:
-        out_sum = torch.empty(shape, dtype=torch.float32, device="cuda")
-        out_count = torch.empty(shape, dtype=torch.int32, device="cuda")
-        mg_mean = torch.empty((w.nperiods, 256), dtype=torch.float32, device="cuda")
-        mg_norm = torch.empty((w.nperiods, 256), dtype=torch.float32, device="cuda")
-    elif not w.fused_normalize:
-        out_sum = torch.empty(shape, dtype=torch.float32, device="cuda")
-        out_count = torch.empty(shape, dtype=torch.int32, device="cuda")
-    ws = torch.empty(gp.gpfc_workspace_bytes(w.ncurves, w.n_total, w.nperiods, w.nbins),
-                     dtype=torch.uint8, device="cuda")
-    gp.gpfc_set_workspace(ws)
-
-    def step():
-        gp.gpfc_make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode, out=periods)
-        gp.gpfc_fold_batch(times, flux, offsets, periods, w.nbins, out_sum=out_sum,
-                           out_count=out_count, out_norm=out_norm)
-        if two_tier:
-            gp.gpfc_merge_equal_count(out_sum, out_count, 256, out_mean=mg_mean, out_norm=mg_norm)
+    gp.gpfc_init()
 
     def barrier():
         torch.cuda.synchronize()
@@ -295,128 +442,66 @@ def gpu_arm(args):
             dist.barrier()
             torch.cuda.synchronize()
 
+    digest = csrc_digest()
+    try:
+        traffic_db = json.load(open(os.path.join(ROOT, "profiles", "r2_traffic.json")))
+    except (OSError, ValueError):
+        traffic_db = {}
     peaks = None
     if rank == 0 and not args.no_peaks:
         peaks = gp.gpfc_measure_peaks()
 
-    for _ in range(args.warmup):
-        step()
-    barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    gp.gpfc_profile(True)
-    e0 = torch.cuda.Event(enable_timing=True)
-    e1 = torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record()
-    barrier()
-    ms = e0.elapsed_time(e1)
-    prof = gp.gpfc_profile_read()
-    gp.gpfc_profile(False)
-    clocks = sampler.stop() if rank == 0 else None
-    ms = max_over_ranks(ms, world, "cuda")
+    # ---- the headline workload
+    w = make_workload(args, rank)
+    run = DeviceRun(gp, torch, w)
+    ms, prof, paths, clocks = run.timed(args.steps, args.warmup, barrier, world,
+                                        ClockSampler(local) if rank == 0 else None)
     pp_step_all = float(w.point_periods) * world
     value = pp_step_all * args.steps / (ms * 1e-3)
+    periods_host = run.periods.cpu().numpy()
+    shape, two_tier = run.shape, run.two_tier
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    roof = roofline_of(w, run, prof, sm_max, peaks, traffic_db, digest) if rank == 0 else None
+    run.free()
 
-    # ---- e2e: the same step through the host-buffer entry points (pinned host memory)
     e2e = None
     if not args.no_e2e:
-        del out_norm, out_sum, out_count
+        e2e = host_e2e(gp, torch, w, shape, max(1, min(args.steps, 3)), barrier, world, two_tier)
         torch.cuda.empty_cache()
-        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-        h_t, h_f, h_o = pin(w.times), pin(w.flux), pin(w.offsets)
-        h_sum = h_cnt = h_norm = None
-        if two_tier:
-            # no host entry point for the two-tier path: the user's calls are the device API
-            # with torch copies (pinned host -> device, merged profiles -> pinned host)
-            h_mean = torch.empty((w.nperiods, 256), dtype=torch.float32, pin_memory=True)
-            h_norm = torch.empty((w.nperiods, 256), dtype=torch.float32, pin_memory=True)
-            d_sum = torch.empty(shape, dtype=torch.float32, device="cuda")
-            d_cnt = torch.empty(shape, dtype=torch.int32, device="cuda")
-        else:
-            h_norm = torch.empty(shape, dtype=torch.float32, pin_memory=True)
-            if not w.fused_normalize:
-                h_sum = torch.empty(shape, dtype=torch.float32, pin_memory=True)
-                h_cnt = torch.empty(shape, dtype=torch.int32, pin_memory=True)
 
-        def step_host():
-            if two_tier:
-                dt_, df_, do_ = (h_t.cuda(non_blocking=True), h_f.cuda(non_blocking=True),
-                                 h_o.cuda(non_blocking=True))
-                per = gp.gpfc_make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode)
-                gp.gpfc_fold_batch(dt_, df_, do_, per, w.nbins, out_sum=d_sum, out_count=d_cnt)
-                m_, n_ = gp.gpfc_merge_equal_count(d_sum, d_cnt, 256)
-                h_mean.copy_(m_.view(-1, 256), non_blocking=True)
-                h_norm.copy_(n_.view(-1, 256), non_blocking=True)
-                torch.cuda.synchronize()
-                return
-            per = gp.gpfc_make_period_grid_host(w.pmin, w.pmax, w.nperiods, w.grid_mode)
-            gp.gpfc_fold_batch_host(h_t, h_f, h_o, per, w.nbins, out_sum=h_sum, out_count=h_cnt,
-                                    out_norm=h_norm)
-
-        nwarm = min(args.warmup, 1)
-        nstep = max(1, min(args.steps, 3))
-        for _ in range(nwarm):
-            step_host()
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(nstep):
-            step_host()
-        barrier()
-        dt = time.perf_counter() - t0
-        dt = max_over_ranks(dt, world, "cuda")
-        nout = int(np.prod(shape)) * 4
-        e2e = {"value": pp_step_all * nstep / dt, "unit": UNIT,
-               "h2d_bytes_per_step": int(w.n_total * 12 + w.offsets.nbytes),
-               "d2h_bytes_per_step": int(nout * (1 if w.fused_normalize else 3) + w.nperiods * 8),
-               "steps": nstep, "api": "gpfc_make_period_grid_host + gpfc_fold_batch_host"}
-        if two_tier:
-            e2e["d2h_bytes_per_step"] = int(2 * w.nperiods * 256 * 4)
-            e2e["api"] = ("torch H2D + gpfc_make_period_grid + gpfc_fold_batch + "
-                          "gpfc_merge_equal_count + torch D2H")
+    # ---- the other BASELINE.json configs (and the paper's own fold), each after its own
+    # warm-up, so that one driver run carries a number for every row of DESIGN.md 7
+    others = []
+    if args.config == 2 and not (args.curves or args.periods or args.no_others) and world == 1:
+        for cid in (1, 3, 4, 5):
+            from paper_2312_02063_b200 import workloads
+            wo = workloads.make(cid)
+            ro = DeviceRun(gp, torch, wo)
+            st = 3
+            ms_o, prof_o, paths_o, _ = ro.timed(st, 3, barrier, 1)
+            rf = roofline_of(wo, ro, prof_o, sm_max, peaks, traffic_db, digest)
+            ent = {"config": workload_desc(wo, args), "value": float(wo.point_periods) * st / (ms_o * 1e-3),
+                   "unit": UNIT, "steps": st, "warmup": 3, "ms_per_step": ms_o / st,
+                   "kernel": rf["kernel"], "kernel_ms": rf["kernel_ms"], "roofline_frac": rf["frac"],
+                   "hbm_frac": rf["hbm_bound"]["frac"], "traffic": rf["traffic"],
+                   "traffic_stale": rf.get("traffic_stale"), "slow_paths": paths_o,
+                   "gpu_launches": int(prof_o["kernel_launches"])}
+            if cid == 5:
+                ent["paper"] = {"workload_s_paper_gpu": 4.32, "workload_s_here_device": ms_o / st * 1e-3,
+                                "cite": "PAPER.md:125-142 Table 1 (RTX 3090 Ti): 0.66 s kernels + 3.66 s "
+                                        "device memory for 70,000 epochs x 100,000 periods"}
+            others.append(ent)
+            ro.free()
+            del wo, ro
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (the fold kernel), DESIGN.md "Roofline"
-    fold_ms = prof["fold_kernel_ms"] / max(prof["fold_launches"], 1)
-    updates = 2.0 * float(w.point_periods)             # one sum + one count update per point-period
-    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
-    peak_nominal = 148 * 32 * sm_max * 1e6              # 32 shared-memory atomic lanes / clk / SM
-    achieved = updates / (fold_ms * 1e-3)
-    out_bytes = float(np.prod(shape)) * 4 * (1 if w.fused_normalize else 3)
-    roof = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_nominal / 1e9,
-            "unit": "G shared-atomic lane-updates/s", "frac": achieved / peak_nominal,
-            "traffic": None,
-            "kernel": "fold_lp_kernel" if w.nbins <= 1024 else "fold_cols_kernel", "kernel_ms": fold_ms,
-            "peak_source": "derived: 148 SMs x 32 lanes/clk x %.0f MHz" % sm_max,
-            "hbm_bound": {"algorithmic_bytes": out_bytes + w.n_total * 12.0,
-                          "achieved_gbs": (out_bytes + w.n_total * 12.0) / (fold_ms * 1e-3) / 1e9}}
-    try:
-        mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-        roof["hbm_bound"]["peak_gbs"] = mp["hbm_gbs"]
-        roof["hbm_bound"]["frac"] = roof["hbm_bound"]["achieved_gbs"] / mp["hbm_gbs"]
-    except (OSError, KeyError, ValueError):
-        roof["hbm_bound"]["peak_gbs"] = 6650.0
-        roof["hbm_bound"]["peak_source"] = "fallback"
-    try:   # DRAM bytes per launch from the committed ncu capture of this workload, if any
-        tj = json.load(open(os.path.join(ROOT, "profiles", "r1_traffic.json"))).get(w.name)
-        if tj and (tj["curves"], tj["nperiods"], tj["nbins"]) == (w.ncurves, w.nperiods, w.nbins):
-            roof["traffic"] = tj["traffic_bytes"]
-            roof["traffic_source"] = "profiles/r1_traffic.json (ncu --set full, commit %s)" % tj["commit"]
-            roof["algorithmic_bytes"] = out_bytes + w.n_total * 12.0
-    except (OSError, KeyError, ValueError):
-        pass
     if peaks:
-        roof["measured_peak"] = peaks["smem_atomic_lane_updates_per_s"] / 1e9
-        roof["frac_of_measured"] = achieved / peaks["smem_atomic_lane_updates_per_s"]
         roof["fp64_pairs_per_s"] = peaks["fp64_mul_add_pairs_per_s"]
-        roof["inner_loop_ceiling_pp_per_s"] = peaks["fold_loop_pp_per_s"]   # fold_lp<0> loop alone
+        roof["inner_loop_ceiling_pp_per_s"] = peaks["fold_loop_pp_per_s"]   # fold_lp loop alone
         roof["alternatives_lane_updates_per_s"] = {
             "cas_float_atomicAdd": peaks["smem_cas_float_lane_updates_per_s"],
             "lds_add_sts_private_rows": peaks["smem_lds_sts_lane_updates_per_s"]}
@@ -425,7 +510,8 @@ def gpu_arm(args):
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": workload_desc(w, args), "clocks": clocks, "roofline": roof,
-           "gpu_launches": int(prof["kernel_launches"])}
+           "gpu_launches": int(prof["kernel_launches"]), "slow_paths": paths,
+           "csrc_digest": digest}
     if two_tier:
         # the paper's profiled fold, same workload, RTX 3090 Ti (context, not target)
         out["vs_baseline"] = value / (70000.0 * 100000.0 / 4.32)
@@ -437,8 +523,9 @@ def gpu_arm(args):
         out["e2e"] = e2e
         if two_tier:
             out["paper"]["workload_s_here_e2e"] = 70000.0 * 100000.0 / e2e["value"]
+    if others:
+        out["other_configs"] = others
     if not args.no_cpu:
-        periods_host = periods.cpu().numpy()
         out["cpu_baseline"] = cpu_baseline(w, periods_host)
     print(json.dumps(out), flush=True)
     if world > 1:

@@ -23,7 +23,16 @@
  *     is enqueued, except the workspace registered with gpfc_set_workspace.
  *   - Device-pointer calls are asynchronous on the calling thread's current
  *     gpfc stream (gpfc_set_stream; default: the legacy default stream) and
- *     never synchronise the host.  *_host calls are synchronous.
+ *     never synchronise the host or any stream; they can be captured in a CUDA
+ *     graph (register a workspace first: gpfc_set_workspace).  *_host calls
+ *     are synchronous.
+ *   - One process may drive several devices: the library keeps its per-device
+ *     state (kernel attributes, SM count) keyed by cudaGetDevice() and sets it
+ *     up on the first call made with that device current, or in gpfc_init().
+ *     Pointers, stream and workspace must belong to the current device.
+ *   - Alignment: times 8 bytes, everything else 4 bytes.  Outputs that are
+ *     16-byte aligned (any torch allocation) are written with vector stores;
+ *     other alignments are accepted and take scalar stores.
  *   - Return value: a gpfc_status (0 = success).  On failure
  *     gpfc_last_error() describes it; outputs are then unspecified.
  *   - Sizes of 0 (n, nperiods, ncurves, nprofiles) are valid no-ops.
@@ -66,6 +75,14 @@ enum { GPFC_GRID_ENDPOINT_INCLUSIVE = 0, GPFC_GRID_ENDPOINT_EXCLUSIVE = 2 };
 /* Library version string (static storage). */
 const char *gpfc_version(void);
 
+/*
+ * Optional: set up the library's per-device state for the CURRENT device now
+ * (opt-in shared-memory attributes of the kernels, SM count).  Every compute
+ * call does the same on its first use of a device; nothing in it touches a
+ * stream, so calling it is never required, not even before graph capture.
+ */
+int gpfc_init(void);
+
 /* Text of the calling thread's last error (static thread-local storage; never NULL). */
 const char *gpfc_last_error(void);
 
@@ -82,6 +99,8 @@ int gpfc_set_stream(void *cuda_stream);
  * uses it has finished) is large enough it is used; otherwise the library
  * allocates and frees scratch stream-ordered (cudaMallocAsync) inside the call.
  * gpfc_set_workspace(NULL, 0) unregisters.  Per-thread, like the stream.
+ * With nbins >= 512 and more than 65,408 samples in the call the bound includes
+ * a 32-bit count overflow area (128 KB per SM, see fold_pk.cu).
  */
 size_t gpfc_workspace_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods, int nbins);
 int gpfc_set_workspace(void *dev_ptr, size_t bytes);
@@ -104,8 +123,15 @@ int gpfc_make_period_grid(double pmin, double pmax, int64_t nperiods, int mode_f
 double gpfc_n_sample(double n_o, double t_window, double l_width);
 
 /*
- * Fold one light curve over a set of trial periods (steps 1-3).
- *   times    device fp64 [n]     sample times (any order, irregular allowed: PAPER.md:334)
+ * Fold one light curve over a set of trial periods (steps 1-3: PAPER.md:87(1), :111
+ * "First" to "Thirdly").
+ *   times    device fp64 [n]     sample times (irregular allowed: PAPER.md:334; any order is
+ *                                accepted and gives the same result, but only time-ordered
+ *                                input is fast: the kernels handle samples in tiles of 128
+ *                                consecutive samples whose time span must stay well below
+ *                                2^20 / nbins periods, other tiles take the exact division
+ *                                for every point-period, ~10x slower; gpfc_path_counters
+ *                                reports how many work items did)
  *   flux     device fp32 [n]     detrended, median-subtracted relative flux
  *   periods  device fp64 [nperiods]
  *   t0       reference epoch subtracted from every time first
@@ -140,7 +166,10 @@ int gpfc_merge_equal_count(const float *sum, const uint32_t *count, int64_t npro
                            int nb2, float *out_mean, float *out_norm);
 
 /*
- * Batched fold, optionally fused with the normalisation.
+ * Batched fold, optionally fused with the normalisation: steps 1-3 and 5 of PAPER.md:111
+ * ("First", "Secondly", "Thirdly", "Lastly") for every (curve, trial period) pair -- the
+ * paper folds one curve at 100,000 periods, 16 at a time (:113-115); here a call folds any
+ * number of curves over a shared grid -- and the noise normalisation of PAPER.md:63.
  *   times, flux  device, curves stored back to back: curve c is samples
  *                offsets[c] .. offsets[c+1]-1
  *   offsets      device int64 [ncurves + 1], non-decreasing, offsets[0] >= 0
@@ -157,6 +186,27 @@ int gpfc_fold_batch(const double *times, const float *flux, const int64_t *offse
                     int64_t ncurves, int64_t n_total, const double *periods,
                     int64_t nperiods, int nbins, const double *t0,
                     float *out_sum, uint32_t *out_count, float *out_norm);
+
+/*
+ * The paper's complete fold, steps 1-5 (Fig. 4): fold at nb1 equal-width
+ * intermediary bins (4096 in the paper), merge them left to right into nb2 bins (256) that
+ * each hold the same number of points, splitting a bin on a boundary pro rata by count
+ * (R18), take the mean of every final bin, and noise-normalise the profile (:63).
+ * Arguments as gpfc_fold_batch (offsets may be NULL when ncurves == 1: the curve is then
+ * times[0 .. n_total)).
+ *   out_mean  device fp32 [ncurves][nperiods][nb2]  mean flux of the final bins   (may be NULL)
+ *   out_norm  device fp32 [ncurves][nperiods][nb2]  the same, scaled to population
+ *             standard deviation 1 about its mean (every final bin counts)       (may be NULL)
+ * For nb1 in {1024, 2048, 4096} and nb2 <= (23 KB * nb1 / 32768) / 8 - 1 (381 for nb1 = 4096)
+ * fold and merge are ONE kernel: the intermediary profile stays in shared memory and the merge
+ * reads the exact integer sums.  Any other (nb1, nb2) folds into a temporary intermediary
+ * profile (stream-ordered allocation, <= 256 MB) and runs gpfc_merge_equal_count on it.
+ * A period that is not finite-positive, or a curve without valid samples, gives zeros.
+ */
+int gpfc_fold_two_tier(const double *times, const float *flux, const int64_t *offsets,
+                       int64_t ncurves, int64_t n_total, const double *periods,
+                       int64_t nperiods, int nb1, int nb2, const double *t0,
+                       float *out_mean, float *out_norm);
 
 /*
  * Host-buffer convenience entry points (the end-to-end path): same
@@ -182,6 +232,19 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
  */
 int gpfc_profile(int enable);
 int gpfc_profile_read(double *fold_kernel_ms, int64_t *fold_launches, int64_t *kernel_launches);
+
+/*
+ * Which slow paths ran since the last gpfc_profile() call (out: host int64[4]):
+ *   [0] fold calls of this thread that used the generic kernel (nbins not a power of two
+ *       in 32 ... 4096: one CTA per (curve, period), true division for every point-period)
+ *   [1] work items (curve x group of periods) of this DEVICE that took the exact division for
+ *       every point-period: unsorted times, tiles spanning huge gaps, periods far below the
+ *       sampling interval
+ *   [2] guard-band re-checks (lane x tile) of this device: normal, ~1e-4 of the tiles
+ *   [3] gpfc_fold_two_tier calls of this thread that could not fuse fold and merge
+ * Synchronises the calling thread's stream.
+ */
+int gpfc_path_counters(int64_t *out);
 
 /*
  * Roofline calibration: runs the library's micro-kernels on

@@ -28,7 +28,7 @@ EXPORTS = [
     "gpfc_set_workspace", "gpfc_make_period_grid", "gpfc_n_sample", "gpfc_fold",
     "gpfc_normalize", "gpfc_fold_batch", "gpfc_make_period_grid_host",
     "gpfc_fold_batch_host", "gpfc_measure_peaks", "gpfc_profile", "gpfc_profile_read",
-    "gpfc_merge_equal_count",
+    "gpfc_merge_equal_count", "gpfc_init", "gpfc_fold_two_tier", "gpfc_path_counters",
 ]
 
 
@@ -68,6 +68,8 @@ def lib() -> ctypes.CDLL:
     L.gpfc_profile.argtypes = [i32]
     L.gpfc_merge_equal_count.argtypes = [vp, vp, i64, i32, i32, vp, vp]
     L.gpfc_profile_read.argtypes = [vp, vp, vp]
+    L.gpfc_fold_two_tier.argtypes = [vp, vp, vp, i64, i64, vp, i64, i32, i32, vp, vp, vp]
+    L.gpfc_path_counters.argtypes = [vp]
     _lib = L
     return L
 
@@ -213,6 +215,40 @@ def gpfc_fold_batch(times, flux, offsets, periods, nbins, t0=None, out_sum=None,
         _dptr(out_count, torch.int32, "out_count"), _dptr(out_norm, torch.float32, "out_norm")),
         "gpfc_fold_batch")
     return out_sum, out_count, out_norm
+
+
+def gpfc_fold_two_tier(times, flux, offsets, periods, nb1, nb2, t0=None, out_mean=None,
+                       out_norm=None, want=("mean", "norm")):
+    """The paper's complete fold: nb1 intermediary bins merged to nb2 equal-count bins.
+    offsets may be None for a single curve.  -> (mean, norm) [ncurves][Np][nb2]."""
+    nc = 1 if offsets is None else offsets.numel() - 1
+    npd, n_total = periods.numel(), times.numel()
+    shape = (nc, npd, int(nb2))
+    if out_mean is None and out_norm is None:
+        if "mean" in want:
+            out_mean = torch.empty(shape, dtype=torch.float32, device=times.device)
+        if "norm" in want:
+            out_norm = torch.empty(shape, dtype=torch.float32, device=times.device)
+    _use_current_stream()
+    _check(lib().gpfc_fold_two_tier(
+        _dptr(times, torch.float64, "times"), _dptr(flux, torch.float32, "flux"),
+        _dptr(offsets, torch.int64, "offsets"), nc, n_total,
+        _dptr(periods, torch.float64, "periods"), npd, int(nb1), int(nb2),
+        _dptr(t0, torch.float64, "t0"), _dptr(out_mean, torch.float32, "out_mean"),
+        _dptr(out_norm, torch.float32, "out_norm")), "gpfc_fold_two_tier")
+    return out_mean, out_norm
+
+
+def gpfc_init() -> None:
+    _check(lib().gpfc_init(), "gpfc_init")
+
+
+def gpfc_path_counters() -> dict:
+    out = (ctypes.c_int64 * 4)()
+    _use_current_stream()
+    _check(lib().gpfc_path_counters(out), "gpfc_path_counters")
+    return {"generic_kernel_calls": out[0], "exact_path_items": out[1],
+            "guard_band_rechecks": out[2], "unfused_two_tier_calls": out[3]}
 
 
 def gpfc_make_period_grid_host(pmin, pmax, nperiods, mode_flags=0):

@@ -3,6 +3,8 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
+#include <new>
 #include <vector>
 
 #include "common.cuh"
@@ -14,9 +16,11 @@ struct ThreadState {
     void *ws = nullptr;
     size_t ws_bytes = 0;
     char err[512] = "";
-    // gpfc_profile: CUDA-event pairs around every fold-kernel launch + launch counter
+    // gpfc_profile: CUDA-event pairs around every fold-kernel launch + launch counters
     bool profiling = false;
-    long long launches = 0;
+    long long launches = 0;           // kernels of this library launched by this thread
+    long long generic_launches = 0;   // ... of which fold_generic_kernel (nbins not a power of two >= 32)
+    long long unfused_two_tier = 0;   // gpfc_fold_two_tier calls that took fold + merge kernels
     std::vector<cudaEvent_t> ev;      // start, stop, start, stop, ...
 };
 
@@ -34,9 +38,60 @@ int cuda_fail(cudaError_t e, const char *where)
     return GPFC_ERR_CUDA;
 }
 
+// ---- per-device state (kernel attributes are per device; so is the SM count)
+constexpr int MAX_DEVICES = 64;
+__device__ unsigned long long g_dev_stats[4];
+
+struct DeviceSlot {
+    bool ready = false;
+    gpfc::DeviceInfo info{};
+};
+DeviceSlot g_dev[MAX_DEVICES];
+std::mutex g_dev_mutex;
+
+}  // namespace
+
+namespace gpfc {
+
+cudaError_t device_info(const DeviceInfo **out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    DeviceSlot &s = g_dev[dev];
+    if (!s.ready) {
+        int n = 0;
+        e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        if (n <= 0) return cudaErrorInvalidDevice;
+        // opt-in dynamic shared memory of every kernel that needs more than 48 KB; none of
+        // these calls touches a stream
+        e = fold_lp_init_device();
+        if (e == cudaSuccess) e = fold_pk_init_device();
+        if (e == cudaSuccess) e = merge_init_device();
+        void *p = nullptr;
+        if (e == cudaSuccess) e = cudaGetSymbolAddress(&p, g_dev_stats);
+        if (e != cudaSuccess) return e;
+        s.info.num_sms = n;
+        s.info.stats = static_cast<unsigned long long *>(p);
+        s.ready = true;
+    }
+    *out = &s.info;
+    return cudaSuccess;
+}
+
+void note_launch(int n) { g_ts.launches += n; }
+
+}  // namespace gpfc
+
+namespace {
+
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
-size_t scratch_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods)
+// scratch of one fold call; `side` > 0 adds the count overflow area of fold_pk.cu
+size_t scratch_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods, size_t side)
 {
     size_t b = 0;
     b += align_up((size_t)n_total * sizeof(double));
@@ -46,7 +101,16 @@ size_t scratch_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods)
     b += align_up((size_t)ncurves * sizeof(gpfc::CurveMeta));
     b += align_up((size_t)nperiods * sizeof(double));
     b += align_up(2 * sizeof(int64_t));   // offsets of the single-curve call
+    b += align_up(side);
     return b + 256;
+}
+
+// curves longer than the flush interval of fold_pk.cu need its 32-bit count overflow area;
+// the curve lengths live on the device, so n_total is the bound the host can test
+size_t side_bytes_for(int64_t n_total, int nbins, int sms)
+{
+    if (!gpfc::fold_pk_handles(nbins) || n_total <= gpfc::fold_pk_flush_samples()) return 0;
+    return gpfc::fold_pk_side_bytes(sms);
 }
 
 __global__ void set_offsets_kernel(int64_t *o, int64_t n)
@@ -55,11 +119,19 @@ __global__ void set_offsets_kernel(int64_t *o, int64_t n)
     o[1] = n;
 }
 
+struct FoldOut {
+    float *sum = nullptr;
+    uint32_t *count = nullptr;
+    float *norm = nullptr;
+    int nb2 = 0;                 // > 0: fused equal-count merge
+    float *mean2 = nullptr;
+    float *norm2 = nullptr;
+};
+
 // The device path shared by every fold entry point.
 int fold_device(const double *times, const float *flux, const int64_t *offsets, int64_t ncurves,
                 int64_t n_total, const double *periods, int64_t nperiods, int nbins,
-                const double *t0v, double t0_scalar, float *out_sum, uint32_t *out_count,
-                float *out_norm)
+                const double *t0v, double t0_scalar, const FoldOut &o)
 {
     if (ncurves < 0 || nperiods < 0 || n_total < 0)
         return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
@@ -68,17 +140,22 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
     if (ncurves == 0 || nperiods == 0) return GPFC_OK;
     if (!periods) return fail(GPFC_ERR_INVALID_ARG, "periods is NULL%s");
     if (n_total > 0 && (!times || !flux)) return fail(GPFC_ERR_INVALID_ARG, "times/flux is NULL%s");
-    if (!out_sum && !out_count && !out_norm) return GPFC_OK;
+    if (o.nb2 == 0 && !o.sum && !o.count && !o.norm) return GPFC_OK;
+    if (o.nb2 > 0 && !o.mean2 && !o.norm2) return GPFC_OK;
 
+    const gpfc::DeviceInfo *di = nullptr;
+    cudaError_t e = gpfc::device_info(&di);
+    if (e != cudaSuccess) return cuda_fail(e, "device initialisation");
     cudaStream_t st = g_ts.stream;
-    size_t need = scratch_bytes(ncurves, n_total, nperiods);
+    const size_t side = side_bytes_for(n_total, nbins, di->num_sms);
+    size_t need = scratch_bytes(ncurves, n_total, nperiods, side);
     char *base = nullptr;
     bool own = false;
     if (g_ts.ws && g_ts.ws_bytes >= need) {
         base = static_cast<char *>(g_ts.ws);
     } else {
         void *p = nullptr;
-        cudaError_t e = cudaMallocAsync(&p, need, st);
+        e = cudaMallocAsync(&p, need, st);
         if (e != cudaSuccess) {
             cuda_fail(e, "scratch allocation");
             return GPFC_ERR_WORKSPACE;
@@ -101,16 +178,16 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
     s.rp = reinterpret_cast<double *>(cur);
     cur += align_up((size_t)nperiods * sizeof(double));
     int64_t *own_off = reinterpret_cast<int64_t *>(cur);
+    cur += align_up(2 * sizeof(int64_t));
+    unsigned *side_p = side ? reinterpret_cast<unsigned *>(cur) : nullptr;
 
-    cudaError_t e = cudaSuccess;
     if (!offsets) {   // single-curve entry point
         set_offsets_kernel<<<1, 1, 0, st>>>(own_off, n_total);
+        gpfc::note_launch();
         offsets = own_off;
-        g_ts.launches += 1;
     }
-    g_ts.launches += 3;   // prep_curves, prep_periods, fold
-    e = gpfc::launch_prep(times, flux, offsets, ncurves, t0v, t0_scalar, periods, nperiods, nbins,
-                          s, st);
+    e = gpfc::launch_prep(times, flux, offsets, ncurves, t0v, t0_scalar, periods, nperiods,
+                          gpfc::fold_rows(nbins), s, st);
     if (e == cudaSuccess) {
         gpfc::FoldArgs a;
         a.u = s.u;
@@ -123,15 +200,25 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
         a.ncurves = ncurves;
         a.nperiods = nperiods;
         a.nbins = nbins;
-        a.out_sum = out_sum;
-        a.out_count = out_count;
-        a.out_norm = out_norm;
-        a.n_min = 0;
-        a.n_max = 0x7fffffff;
+        a.out_sum = o.sum;
+        a.out_count = o.count;
+        a.out_norm = o.norm;
+        a.vec_ok = ((reinterpret_cast<uintptr_t>(o.sum) | reinterpret_cast<uintptr_t>(o.count) |
+                     reinterpret_cast<uintptr_t>(o.norm)) & 15) == 0;
+        a.nb2 = o.nb2;
+        a.out_mean2 = o.mean2;
+        a.out_norm2 = o.norm2;
+        a.side = side_p;
+        a.stats = di->stats;
+        if (!gpfc::fold_lp_handles(nbins) && !gpfc::fold_pk_handles(nbins)) g_ts.generic_launches += 1;
         cudaEvent_t e0 = nullptr, e1 = nullptr;
-        if (g_ts.profiling && cudaEventCreate(&e0) == cudaSuccess &&
-            cudaEventCreate(&e1) == cudaSuccess)
-            cudaEventRecord(e0, st);
+        if (g_ts.profiling) {
+            if (cudaEventCreate(&e0) == cudaSuccess && cudaEventCreate(&e1) != cudaSuccess) {
+                cudaEventDestroy(e0);
+                e0 = nullptr;
+            }
+            if (e0 && e1) cudaEventRecord(e0, st);
+        }
         e = gpfc::launch_fold(a, st);
         if (e0 && e1) {
             cudaEventRecord(e1, st);
@@ -147,13 +234,27 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
     return GPFC_OK;
 }
 
+int check_bins(int nb)
+{
+    if (nb < 1 || nb > GPFC_MAX_NBINS) return fail(GPFC_ERR_UNSUPPORTED, "bin counts must be in [1, 4096]%s");
+    return GPFC_OK;
+}
+
 }  // namespace
 
 extern "C" {
 
-const char *gpfc_version(void) { return "gpfc-b200 0.1 (sm_100a)"; }
+const char *gpfc_version(void) { return "gpfc-b200 0.2 (sm_100a)"; }
 
 const char *gpfc_last_error(void) { return g_ts.err; }
+
+int gpfc_init(void)
+{
+    const gpfc::DeviceInfo *di = nullptr;
+    cudaError_t e = gpfc::device_info(&di);
+    if (e != cudaSuccess) return cuda_fail(e, "gpfc_init");
+    return GPFC_OK;
+}
 
 int gpfc_set_stream(void *cuda_stream)
 {
@@ -163,9 +264,10 @@ int gpfc_set_stream(void *cuda_stream)
 
 size_t gpfc_workspace_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods, int nbins)
 {
-    (void)nbins;
     if (ncurves < 0 || n_total < 0 || nperiods < 0) return 0;
-    return scratch_bytes(ncurves, n_total, nperiods);
+    // the count overflow area is sized for the largest SM count of the family (no device query:
+    // this call works without a GPU)
+    return scratch_bytes(ncurves, n_total, nperiods, side_bytes_for(n_total, nbins, 160));
 }
 
 int gpfc_set_workspace(void *dev_ptr, size_t bytes)
@@ -196,7 +298,6 @@ int gpfc_make_period_grid(double pmin, double pmax, int64_t nperiods, int mode_f
     if (!periods_out) return fail(GPFC_ERR_INVALID_ARG, "periods_out is NULL%s");
     cudaError_t e = gpfc::launch_grid(pmin, pmax, nperiods, mode_flags, periods_out, g_ts.stream);
     if (e != cudaSuccess) return cuda_fail(e, "grid launch");
-    g_ts.launches += 1;
     return GPFC_OK;
 }
 
@@ -204,21 +305,21 @@ int gpfc_fold(const double *times, const float *flux, int64_t n, const double *p
               int64_t nperiods, int nbins, double t0, float *out_sum, uint32_t *out_count)
 {
     if (n < 0) return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
-    return fold_device(times, flux, nullptr, 1, n, periods, nperiods, nbins, nullptr, t0, out_sum,
-                       out_count, nullptr);
+    FoldOut o;
+    o.sum = out_sum;
+    o.count = out_count;
+    return fold_device(times, flux, nullptr, 1, n, periods, nperiods, nbins, nullptr, t0, o);
 }
 
 int gpfc_normalize(const float *sum, const uint32_t *count, int64_t nprofiles, int nbins,
                    float *out_norm)
 {
     if (nprofiles < 0) return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
-    if (nbins < 1 || nbins > GPFC_MAX_NBINS)
-        return fail(GPFC_ERR_UNSUPPORTED, "nbins must be in [1, 4096]%s");
+    if (check_bins(nbins) != GPFC_OK) return GPFC_ERR_UNSUPPORTED;
     if (nprofiles == 0) return GPFC_OK;
     if (!sum || !count || !out_norm) return fail(GPFC_ERR_INVALID_ARG, "NULL pointer%s");
     cudaError_t e = gpfc::launch_normalize(sum, count, nprofiles, nbins, out_norm, g_ts.stream);
     if (e != cudaSuccess) return cuda_fail(e, "normalize launch");
-    g_ts.launches += 1;
     return GPFC_OK;
 }
 
@@ -226,14 +327,14 @@ int gpfc_merge_equal_count(const float *sum, const uint32_t *count, int64_t npro
                            int nb2, float *out_mean, float *out_norm)
 {
     if (nprofiles < 0) return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
-    if (nb1 < 1 || nb1 > GPFC_MAX_NBINS || nb2 < 1 || nb2 > GPFC_MAX_NBINS)
-        return fail(GPFC_ERR_UNSUPPORTED, "nb1 and nb2 must be in [1, 4096]%s");
+    if (check_bins(nb1) != GPFC_OK || check_bins(nb2) != GPFC_OK) return GPFC_ERR_UNSUPPORTED;
     if (nprofiles == 0) return GPFC_OK;
     if (!sum || !count || (!out_mean && !out_norm)) return fail(GPFC_ERR_INVALID_ARG, "NULL pointer%s");
-    cudaError_t e = gpfc::launch_merge(sum, count, nprofiles, nb1, nb2, out_mean, out_norm,
-                                       g_ts.stream);
+    const gpfc::DeviceInfo *di = nullptr;
+    cudaError_t e = gpfc::device_info(&di);
+    if (e == cudaSuccess)
+        e = gpfc::launch_merge(sum, count, nprofiles, nb1, nb2, out_mean, out_norm, g_ts.stream);
     if (e != cudaSuccess) return cuda_fail(e, "merge launch");
-    g_ts.launches += 1;
     return GPFC_OK;
 }
 
@@ -243,8 +344,66 @@ int gpfc_fold_batch(const double *times, const float *flux, const int64_t *offse
                     float *out_norm)
 {
     if (ncurves > 0 && !offsets) return fail(GPFC_ERR_INVALID_ARG, "offsets is NULL%s");
-    return fold_device(times, flux, offsets, ncurves, n_total, periods, nperiods, nbins, t0, 0.0,
-                       out_sum, out_count, out_norm);
+    FoldOut o;
+    o.sum = out_sum;
+    o.count = out_count;
+    o.norm = out_norm;
+    return fold_device(times, flux, offsets, ncurves, n_total, periods, nperiods, nbins, t0, 0.0, o);
+}
+
+int gpfc_fold_two_tier(const double *times, const float *flux, const int64_t *offsets,
+                       int64_t ncurves, int64_t n_total, const double *periods,
+                       int64_t nperiods, int nb1, int nb2, const double *t0, float *out_mean,
+                       float *out_norm)
+{
+    if (ncurves < 0 || nperiods < 0 || n_total < 0)
+        return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
+    if (check_bins(nb1) != GPFC_OK || check_bins(nb2) != GPFC_OK) return GPFC_ERR_UNSUPPORTED;
+    if (ncurves > 1 && !offsets) return fail(GPFC_ERR_INVALID_ARG, "offsets is NULL%s");
+    if (ncurves == 0 || nperiods == 0 || (!out_mean && !out_norm)) return GPFC_OK;
+    if (gpfc::fold_pk_can_merge(nb1, nb2)) {
+        // fused: the nb1 intermediary bins never leave shared memory
+        FoldOut o;
+        o.nb2 = nb2;
+        o.mean2 = out_mean;
+        o.norm2 = out_norm;
+        return fold_device(times, flux, offsets, ncurves, n_total, periods, nperiods, nb1, t0, 0.0, o);
+    }
+    // any other (nb1, nb2): fold into a temporary intermediary profile, chunk by chunk over the
+    // period axis (<= 256 MB of sums + counts at a time), then the stand-alone merge kernel
+    if (!periods) return fail(GPFC_ERR_INVALID_ARG, "periods is NULL%s");
+    g_ts.unfused_two_tier += 1;
+    cudaStream_t st = g_ts.stream;
+    int64_t chunk = (int64_t)((size_t)(128u << 20) / ((size_t)nb1 * 4));
+    if (chunk < 1) chunk = 1;
+    if (chunk > nperiods) chunk = nperiods;
+    char *tmp = nullptr;
+    const size_t arr = align_up((size_t)chunk * (size_t)nb1 * 4);
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&tmp), 2 * arr + 16 * (size_t)(ncurves + 1), st);
+    if (e != cudaSuccess) {
+        cuda_fail(e, "intermediary profile allocation");
+        return GPFC_ERR_WORKSPACE;
+    }
+    float *t_sum = reinterpret_cast<float *>(tmp);
+    uint32_t *t_cnt = reinterpret_cast<uint32_t *>(tmp + arr);
+    int rc = GPFC_OK;
+    for (int64_t c = 0; c < ncurves && rc == GPFC_OK; ++c) {
+        for (int64_t j0 = 0; j0 < nperiods && rc == GPFC_OK; j0 += chunk) {
+            const int64_t nj = (nperiods - j0 < chunk) ? nperiods - j0 : chunk;
+            FoldOut o;
+            o.sum = t_sum;
+            o.count = t_cnt;
+            rc = fold_device(times, flux, offsets ? offsets + c : nullptr, 1, n_total, periods + j0, nj,
+                             nb1, t0 ? t0 + c : nullptr, 0.0, o);
+            if (rc != GPFC_OK) break;
+            e = gpfc::launch_merge(t_sum, t_cnt, nj, nb1, nb2,
+                                   out_mean ? out_mean + ((size_t)c * nperiods + j0) * nb2 : nullptr,
+                                   out_norm ? out_norm + ((size_t)c * nperiods + j0) * nb2 : nullptr, st);
+            if (e != cudaSuccess) rc = cuda_fail(e, "merge launch");
+        }
+    }
+    cudaFreeAsync(tmp, st);
+    return rc;
 }
 
 int gpfc_make_period_grid_host(double pmin, double pmax, int64_t nperiods, int mode_flags,
@@ -259,7 +418,6 @@ int gpfc_make_period_grid_host(double pmin, double pmax, int64_t nperiods, int m
     cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&d), (size_t)nperiods * 8, st);
     if (e != cudaSuccess) return cuda_fail(e, "grid alloc");
     e = gpfc::launch_grid(pmin, pmax, nperiods, mode_flags, d, st);
-    g_ts.launches += 1;
     if (e == cudaSuccess)
         e = cudaMemcpyAsync(periods_out, d, (size_t)nperiods * 8, cudaMemcpyDeviceToHost, st);
     cudaFreeAsync(d, st);
@@ -346,11 +504,12 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
         if (e != cudaSuccess) break;
         // the prepass scratch covers the samples offsets[c0] .. offsets[c0 + nc]: pass the
         // whole arrays (offsets are absolute) and size the scratch by n_total
+        FoldOut o;
+        o.sum = reinterpret_cast<float *>(slab[s][0]);
+        o.count = reinterpret_cast<uint32_t *>(slab[s][1]);
+        o.norm = reinterpret_cast<float *>(slab[s][2]);
         rc = fold_device(d_t, d_f, d_o + c0, nc, n_total, d_p, nperiods, nbins,
-                         d_t0 ? d_t0 + c0 : nullptr, 0.0,
-                         reinterpret_cast<float *>(slab[s][0]),
-                         reinterpret_cast<uint32_t *>(slab[s][1]),
-                         reinterpret_cast<float *>(slab[s][2]));
+                         d_t0 ? d_t0 + c0 : nullptr, 0.0, o);
         if (rc != GPFC_OK) break;
         e = cudaEventRecord(done[s], st);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, done[s], 0);
@@ -383,7 +542,12 @@ int gpfc_profile(int enable)
     for (cudaEvent_t ev : g_ts.ev) cudaEventDestroy(ev);
     g_ts.ev.clear();
     g_ts.launches = 0;
+    g_ts.generic_launches = 0;
+    g_ts.unfused_two_tier = 0;
     g_ts.profiling = enable != 0;
+    const gpfc::DeviceInfo *di = nullptr;
+    if (gpfc::device_info(&di) == cudaSuccess)
+        cudaMemsetAsync(di->stats, 0, 4 * sizeof(unsigned long long), g_ts.stream);
     return GPFC_OK;
 }
 
@@ -400,6 +564,23 @@ int gpfc_profile_read(double *fold_kernel_ms, int64_t *fold_launches, int64_t *k
     if (fold_kernel_ms) *fold_kernel_ms = total;
     if (fold_launches) *fold_launches = (int64_t)(g_ts.ev.size() / 2);
     if (kernel_launches) *kernel_launches = g_ts.launches;
+    return GPFC_OK;
+}
+
+int gpfc_path_counters(int64_t *out)
+{
+    if (!out) return fail(GPFC_ERR_INVALID_ARG, "out is NULL%s");
+    out[0] = g_ts.generic_launches;
+    out[1] = out[2] = 0;
+    out[3] = g_ts.unfused_two_tier;
+    const gpfc::DeviceInfo *di = nullptr;
+    cudaError_t e = gpfc::device_info(&di);
+    unsigned long long h[4] = {0, 0, 0, 0};
+    if (e == cudaSuccess) e = cudaStreamSynchronize(g_ts.stream);
+    if (e == cudaSuccess) e = cudaMemcpy(h, di->stats, sizeof(h), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(e, "gpfc_path_counters");
+    out[1] = (int64_t)h[0];
+    out[2] = (int64_t)h[1];
     return GPFC_OK;
 }
 

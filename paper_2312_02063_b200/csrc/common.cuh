@@ -33,6 +33,12 @@ struct CurveMeta {
     double umax;
     double span_max;   // largest tile span of the curve
     double pivot;      // mean of the centred, quantised flux: (sum q) 2^-s / n_valid
+    // Samples with u == 0 exactly (t == t0: the first sample of a curve whose times start at
+    // t0) have phase 0 and bin 0 at EVERY period, and would sit in the guard band of every
+    // (tile, period).  The prepass keeps up to 255 of them out of the sample arrays; the fold
+    // epilogues add them to bin 0: n_zero points with fixed-point flux sum q_zero.
+    int n_zero;
+    int q_zero;
 };
 
 // Scratch carved out of the workspace for one gpfc_fold_batch call.
@@ -43,7 +49,8 @@ struct Scratch {
     TileInfo *tiles;   // [n_total / GPFC_TILE + ncurves + 1]
     CurveMeta *meta;   // [ncurves]
     double *rp;        // [nperiods] RN(1/P) * rows, NaN for a period that is not finite-positive;
-                       // rows = 256 for power-of-two nbins in [32, 256] (lane-period kernel), else nbins
+                       // rows = fold_rows(nbins): 256 for nbins in {32..256}, 1024 for {512, 1024},
+                       // else nbins
 };
 
 struct FoldArgs {
@@ -60,8 +67,25 @@ struct FoldArgs {
     float *out_sum;
     uint32_t *out_count;
     float *out_norm;
-    int n_min, n_max;   // a launch handles the curves with n_min <= n_valid <= n_max
+    int vec_ok;                   // every non-NULL output above is 16-byte aligned (vector stores)
+    // fused equal-count merge (fold_pk.cu): nb2 > 0 replaces the three outputs above
+    int nb2;
+    float *out_mean2;             // [curve][period][nb2]
+    float *out_norm2;             // [curve][period][nb2]
+    unsigned *side;               // fold_pk.cu: 32-bit count overflow area, 32768 words per CTA, or NULL
+    unsigned long long *stats;    // device counters (DeviceInfo::stats), or NULL
 };
+
+// Per-device state, initialised on first use of a device by any thread (api.cu): kernel
+// attributes (opt-in dynamic shared memory) are per device, so is the SM count.  Nothing here
+// synchronises a stream or the host.
+struct DeviceInfo {
+    int num_sms;
+    unsigned long long *stats;    // device counters: [0] work items folded with the exact formula
+                                  // for every point-period, [1] guard-band re-checks (lane x tile)
+};
+cudaError_t device_info(const DeviceInfo **out);
+void note_launch(int n = 1);      // per-thread kernel-launch counter (gpfc_profile_read)
 
 // ---- exact bin of one sample (-1 = skip the sample, reading R20): the formula of include/gpfc.h, every operation
 // rounded once (intrinsics, so nothing can be contracted into an FMA).
@@ -159,17 +183,25 @@ __device__ __forceinline__ void emit_profile(unsigned long long *slots, int nbin
     }
 }
 
-// launchers (defined in the .cu files)
+// launchers (defined in the .cu files).  Every launch_* counts its kernels with note_launch().
 cudaError_t launch_prep(const double *times, const float *flux, const int64_t *offsets,
                         long long ncurves, const double *t0, double t0_scalar,
-                        const double *periods, long long nperiods, int nbins, Scratch s,
+                        const double *periods, long long nperiods, int rows, Scratch s,
                         cudaStream_t st);
+int fold_rows(int nbins);         // fold.cu: resolution the fold kernel for `nbins` works at
 cudaError_t launch_fold(const FoldArgs &a, cudaStream_t st);
-cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st);   // fold_lp.cu: nbins in {32,64,128,256}
-cudaError_t launch_fold_generic(const FoldArgs &a, cudaStream_t st);   // fold.cu: any nbins, exact formula
+cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st, int sms);   // fold_lp.cu: nbins 32..256
+cudaError_t launch_fold_pk(const FoldArgs &a, cudaStream_t st, int sms);   // fold_pk.cu: nbins 512..4096
+cudaError_t launch_fold_generic(const FoldArgs &a, cudaStream_t st, int sms);   // fold.cu: any nbins
 bool fold_lp_handles(int nbins);
-int fold_lp_rows(int nbins);   // fold resolution of the lane-period kernel (256 or 1024)
-int num_sms();
+bool fold_pk_handles(int nbins);
+int fold_pk_rows(int nbins);
+bool fold_pk_can_merge(int nbins, int nb2);      // the fused equal-count merge fits in shared memory
+size_t fold_pk_side_bytes(int sms);
+long long fold_pk_flush_samples();               // curves longer than this need FoldArgs::side
+cudaError_t fold_lp_init_device();
+cudaError_t fold_pk_init_device();
+cudaError_t merge_init_device();
 cudaError_t launch_normalize(const float *sum, const uint32_t *count, long long nprofiles,
                              int nbins, float *out, cudaStream_t st);
 cudaError_t launch_merge(const float *sum, const uint32_t *count, long long nprofiles, int nb1,

@@ -28,55 +28,39 @@
 //   (exact: floor(phi * 256) >> k == floor(phi * (256 >> k))).
 // * Epilogue: lane l walks ITS periods' rows (conflict-free), so mean / std need no
 //   cross-lane reduction; every lane writes 32-byte sectors (8 bins) of its own rows.
-#include <mutex>
-
 #include "common.cuh"
 
 namespace gpfc {
 
 namespace {
 
-constexpr int LP_MAX_WARPS = 24;              // largest variant: sizes the staging area
-constexpr int LP_EPI_WARPS = 8;               // sizes the statistics partials: (warps / R) * 32 R <= 8 * 96
+constexpr int LP_R = 3;                       // periods per lane
+constexpr int LP_ROWLOG = 8, LP_ROWS = 256;
+constexpr int LP_THREADS = 768, LP_WARPS = LP_THREADS / 32;
+constexpr int LP_GROUP = 32 * LP_R;           // periods per work item
+constexpr int LP_WPR = LP_WARPS / LP_R;       // epilogue: warps per period slot
 constexpr int LP_GRAN = 64;                   // samples per staging granule
-constexpr unsigned LP_SMEM_BASE = 0x400;      // shared-window address of dynamic shared memory
 
-// Two variants of the kernel:
-//   VAR 0: 256 rows, R = 3 periods per lane, histogram [r][row][sum|count][lane] (nbins 32..256)
-//   VAR 1: 1024 rows, R = 1, sums [row][lane] (128 KB) and PACKED counts [row & 511][lane]
-//          (64 KB): the low half-word counts rows k and k + 512 together, the high half-word
-//          counts row k + 512, so a curve may have at most 65,535 valid samples
-//          (nbins 512, 1024; longer curves are left to fold_generic_kernel).
-template <int VAR> struct LpV;
-template <> struct LpV<0> {
-    static constexpr int R = 3, ROWLOG = 8, THREADS = 768;
-    static constexpr bool PACKED = false;
-};
-template <> struct LpV<1> {
-    static constexpr int R = 1, ROWLOG = 10, THREADS = 768;
-    static constexpr bool PACKED = true;
-};
-constexpr int LP_GROUP_MAX = 96;              // periods per work item, largest variant
-constexpr int LP_PACKED_MAX_N = 65535;
-
-constexpr int LP_HIST_BYTES = 196608;         // both variants
-constexpr int LP_CNT1_OFF = 131072;           // VAR 1: byte offset of the packed counts
+constexpr int LP_HIST_BYTES = 196608;         // [r][row][sum|count][lane] 32-bit words
 // scratch after the histograms: sample staging during the fold, statistics partials in the
 // epilogue (the two never live at the same time)
 constexpr int LP_STAGE_OFF = LP_HIST_BYTES;                   // int2 [warps][LP_GRAN]
-constexpr int LP_PS1_OFF = LP_HIST_BYTES;                     // double [LP_EPI_WARPS][GROUP]
-constexpr int LP_PS2_OFF = LP_PS1_OFF + LP_EPI_WARPS * LP_GROUP_MAX * 8;
-constexpr int LP_PKK_OFF = LP_PS2_OFF + LP_EPI_WARPS * LP_GROUP_MAX * 8;   // int [LP_EPI_WARPS][GROUP]
-constexpr int LP_MU_OFF = LP_PKK_OFF + LP_EPI_WARPS * LP_GROUP_MAX * 4;    // double [GROUP]
-constexpr int LP_ISD_OFF = LP_MU_OFF + LP_GROUP_MAX * 8;                   // double [GROUP]
-constexpr int LP_KK_OFF = LP_ISD_OFF + LP_GROUP_MAX * 8;                   // int [GROUP]
-constexpr int LP_CTR_OFF = LP_KK_OFF + LP_GROUP_MAX * 4;
+constexpr int LP_PS1_OFF = LP_HIST_BYTES;                     // double [LP_WPR][GROUP]
+constexpr int LP_PS2_OFF = LP_PS1_OFF + LP_WPR * LP_GROUP * 8;
+constexpr int LP_PKK_OFF = LP_PS2_OFF + LP_WPR * LP_GROUP * 8;   // int [LP_WPR][GROUP]
+constexpr int LP_MU_OFF = LP_PKK_OFF + LP_WPR * LP_GROUP * 4;    // double [GROUP]
+constexpr int LP_ISD_OFF = LP_MU_OFF + LP_GROUP * 8;             // double [GROUP]
+constexpr int LP_KK_OFF = LP_ISD_OFF + LP_GROUP * 8;             // int [GROUP]
+constexpr int LP_CTR_OFF = LP_KK_OFF + LP_GROUP * 4;
 constexpr int LP_SMEM_BYTES = LP_CTR_OFF + 16;
 static_assert(LP_SMEM_BYTES <= 227 * 1024, "shared memory budget");
 static_assert(GPFC_TILE == 2 * LP_GRAN, "half-tile work units are one staging granule");
-static_assert(LP_MAX_WARPS * LP_GRAN * 8 <= LP_MU_OFF - LP_STAGE_OFF, "staging fits in the scratch");
+static_assert(LP_WARPS * LP_GRAN * 8 <= LP_MU_OFF - LP_STAGE_OFF, "staging fits in the scratch");
+static_assert(LP_WARPS % LP_R == 0, "warps per period slot");
 
-// shared-memory reductions with an immediate offset: ATOMS.ADD / ATOMS.POPC.INC
+// shared-memory reductions with an immediate offset: ATOMS.ADD / ATOMS.POPC.INC [R + UR + imm].
+// `addr` carries the shared-window address of the histogram (__cvta_generic_to_shared), which
+// ptxas keeps in a uniform register: the window base is never assumed.
 template <int IMM>
 __device__ __forceinline__ void red_add(unsigned addr, int v)
 {
@@ -88,63 +72,17 @@ __device__ __forceinline__ void red_inc(unsigned addr)
     asm volatile("red.shared.add.u32 [%0+%1], 1;" ::"r"(addr), "n"(IMM) : "memory");
 }
 
-// word index of (r, row, array, lane) in the unpacked histogram [r][row][sum|count][lane]
-template <int VAR>
+// word index of (r, row, array, lane) in the histogram [r][row][sum|count][lane]
 __device__ __forceinline__ int hidx(int r, int row, int arr, int lane)
 {
-    return r * (64 << LpV<VAR>::ROWLOG) + row * 64 + arr * 32 + lane;
-}
-
-// word index of the sum of (r, row, lane)
-template <int VAR>
-__device__ __forceinline__ int sum_word(int r, int row, int lane)
-{
-    if (!LpV<VAR>::PACKED) return hidx<VAR>(r, row, 0, lane);
-    return row * 32 + lane;
-}
-
-// word index and half-word of the packed count of (r, row, lane), and the value that adds
-// one sample to it
-template <int VAR>
-__device__ __forceinline__ int cnt_word(int r, int row, int lane)
-{
-    return LP_CNT1_OFF / 4 + (row & 511) * 32 + lane;
-}
-template <int VAR>
-__device__ __forceinline__ unsigned cnt_unit(int r, int row)
-{
-    return 1u + ((unsigned)(row >> 9) << 16);   // low half counts both rows
+    return r * (64 * LP_ROWS) + row * 64 + arr * 32 + lane;
 }
 
 // generic (slow-path) update of one sample: move = +1 adds it to `row`, -1 removes it
-template <int VAR>
 __device__ __forceinline__ void hist_update(unsigned *H, int r, int row, int lane, int q, int move)
 {
-    atomicAdd(&H[sum_word<VAR>(r, row, lane)], (unsigned)(move * q));
-    if (!LpV<VAR>::PACKED)
-        atomicAdd(&H[hidx<VAR>(r, row, 1, lane)], (unsigned)move);
-    else
-        atomicAdd(&H[cnt_word<VAR>(r, row, lane)], (unsigned)move * cnt_unit<VAR>(r, row));
-}
-
-// one bin = M consecutive rows: exact sum and count
-template <int VAR>
-__device__ __forceinline__ void read_bin(const unsigned *H, int r, int row0, int M, int lane, int &S,
-                                         unsigned &c)
-{
-    S = 0;
-    c = 0;
-#pragma unroll 1
-    for (int jj = 0; jj < M; ++jj) {
-        const int row = row0 + jj;
-        S += (int)H[sum_word<VAR>(r, row, lane)];
-        if (!LpV<VAR>::PACKED) {
-            c += H[hidx<VAR>(r, row, 1, lane)];
-        } else {
-            const unsigned w = H[cnt_word<VAR>(r, row, lane)];
-            c += (row >> 9) ? (w >> 16) : ((w & 0xffffu) - (w >> 16));
-        }
-    }
+    atomicAdd(&H[hidx(r, row, 0, lane)], (unsigned)(move * q));
+    atomicAdd(&H[hidx(r, row, 1, lane)], (unsigned)move);
 }
 
 // sq / c for a count c in [1, 2^32): reciprocal from an fp32 seed + two Newton steps
@@ -160,63 +98,47 @@ __device__ __forceinline__ double div_by_count(double sq, unsigned c)
     return __fma_rn(__fma_rn(-q0, cd, sq), r, q0);
 }
 
-// the constant 1 in a register the compiler cannot fold, so that (t7 & 0x10000) | 1 is ONE LOP3
-__device__ __forceinline__ unsigned opaque_one()
-{
-    unsigned one;
-    asm volatile("mov.u32 %0, 1;" : "=r"(one));
-    return one;
-}
+// Shared-window address of dynamic shared memory on sm_100a (the first KB of the window is the
+// driver's): with this value the histogram offsets are instruction immediates.  The kernel
+// compares it with the real address and takes the register-base code path if they differ
+// (one more integer add per point-period, same results), so nothing depends on it.
+constexpr unsigned LP_WINDOW_BASE = 0x400;
 
-template <int VAR, int r>
+template <int r, bool IMM>
 __device__ __forceinline__ void pp_update(double v, int q, double rp, double C, unsigned lane4,
-                                          unsigned one, unsigned &gmin)
+                                          unsigned sbase, unsigned &gmin)
 {
     double m = __fma_rd(v, rp, C);
     unsigned lo = (unsigned)__double2loint(m), hi = (unsigned)__double2hiint(m);
     gmin = min(gmin, lo);
-    if (VAR == 0) {
-        unsigned addr = __byte_perm(lane4, hi, 0x3240);      // (row << 8) | (lane << 2)
-        red_add<(int)LP_SMEM_BASE + r * 65536>(addr, q);
-        red_inc<(int)LP_SMEM_BASE + r * 65536 + 128>(addr);
+    unsigned addr = __byte_perm(lane4, hi, 0x3240);      // (row << 8) | (lane << 2)
+    if (IMM) {
+        red_add<(int)LP_WINDOW_BASE + r * 65536>(addr, q);
+        red_inc<(int)LP_WINDOW_BASE + r * 65536 + 128>(addr);
     } else {
-        const unsigned t7 = hi << 7;                         // row << 7 (+ junk above bit 16)
-        const unsigned saddr = (t7 & 0x1ff80u) | lane4;      // row * 128 + lane * 4
-        const unsigned caddr = (t7 & 0x0ff80u) | lane4;      // (row & 511) * 128 + lane * 4
-        const unsigned val = (t7 & 0x10000u) | one;          // 1 + ((row >> 9) << 16)
-        red_add<(int)LP_SMEM_BASE>(saddr, q);
-        red_add<(int)LP_SMEM_BASE + LP_CNT1_OFF>(caddr, (int)val);
+        addr += sbase;
+        red_add<r * 65536>(addr, q);
+        red_inc<r * 65536 + 128>(addr);
     }
 }
 
-template <int VAR, int r0>
+template <int r0, bool IMM>
 struct ForR {
-    static constexpr int R = LpV<VAR>::R;
-    __device__ __forceinline__ static void run(double v, int q, const double (&rp)[R],
-                                               const double (&C)[R], unsigned lane4,
-                                               unsigned one, unsigned (&gmin)[R])
+    __device__ __forceinline__ static void run(double v, int q, const double (&rp)[LP_R],
+                                               const double (&C)[LP_R], unsigned lane4,
+                                               unsigned sbase, unsigned (&gmin)[LP_R])
     {
-        if constexpr (r0 < R) {
-            pp_update<VAR, r0>(v, q, rp[r0], C[r0], lane4, one, gmin[r0]);
-            ForR<VAR, r0 + 1>::run(v, q, rp, C, lane4, one, gmin);
+        if constexpr (r0 < LP_R) {
+            pp_update<r0, IMM>(v, q, rp[r0], C[r0], lane4, sbase, gmin[r0]);
+            ForR<r0 + 1, IMM>::run(v, q, rp, C, lane4, sbase, gmin);
         }
     }
 };
 
-template <int VAR>
-__global__ void __launch_bounds__(LpV<VAR>::THREADS, 1)
-fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
+template <bool IMM>
+__device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroups, long long nitems,
+                                             unsigned char *smem, unsigned sbase)
 {
-    using V = LpV<VAR>;
-    constexpr int LP_R = V::R, LP_ROWS = 1 << V::ROWLOG, LP_GROUP = 32 * V::R;
-    constexpr int LP_THREADS = V::THREADS, LP_WARPS = V::THREADS / 32;
-    static_assert(LP_WARPS <= LP_MAX_WARPS, "staging area");
-    static_assert((LP_WARPS / LP_R) * LP_GROUP <= LP_EPI_WARPS * LP_GROUP_MAX, "statistics partials");
-    extern __shared__ __align__(1024) unsigned char smem[];
-    if (probe) {   // report where dynamic shared memory starts (host checks LP_SMEM_BASE once)
-        if (threadIdx.x == 0 && blockIdx.x == 0) *probe = (unsigned)__cvta_generic_to_shared(smem);
-        return;
-    }
     unsigned *H = reinterpret_cast<unsigned *>(smem);
     double *ps1 = reinterpret_cast<double *>(smem + LP_PS1_OFF);
     double *ps2 = reinterpret_cast<double *>(smem + LP_PS2_OFF);
@@ -228,25 +150,23 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned lane4 = (unsigned)lane << 2;
-    const unsigned one = opaque_one();
     int4 *stage = reinterpret_cast<int4 *>(smem + LP_STAGE_OFF) + warp * (LP_GRAN / 2);
     for (int i = tid; i < LP_HIST_BYTES / 4; i += LP_THREADS) H[i] = 0u;
     if (tid == 0) *ctr = 0;
     __syncthreads();
 
     const int nb = a.nbins;                      // power of two, 32 <= nb <= LP_ROWS
-    const int mshift = V::ROWLOG - (31 - __clz(nb));   // rows merged per bin = 1 << mshift
+    const int mshift = LP_ROWLOG - (31 - __clz(nb));   // rows merged per bin = 1 << mshift
     const int M = 1 << mshift;
-    // 1.5 * 2^(52 + ROWLOG): ulp = LP_ROWS
-    const double M2 = (V::ROWLOG == 8) ? 1729382256910270464.0 : 6917529027641081856.0;
+    const double M2 = 1729382256910270464.0;     // 1.5 * 2^(52 + ROWLOG): ulp = LP_ROWS
     const bool want_norm = a.out_norm != nullptr;
+    const bool vec = a.vec_ok != 0;
 
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const long long curve = item / ngroups;
         const long long p0 = (item - curve * ngroups) * LP_GROUP;
         const CurveMeta cm = a.meta[curve];
         const int n = cm.n_valid;
-        if (n < a.n_min || n > a.n_max) continue;      // another launch owns this curve
         const int ntiles = (n + GPFC_TILE - 1) / GPFC_TILE;
 
         // this lane's periods
@@ -323,17 +243,17 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
 #pragma unroll 1
                         for (int s = 0; s < LP_GRAN / 2; s += 2) {
                             const int4 ra = stage[s], rb = stage[s + 1];
-                            ForR<VAR, 0>::run((double)(unsigned)ra.x, ra.y, rps, C, lane4, one, gmin);
-                            ForR<VAR, 0>::run((double)(unsigned)ra.z, ra.w, rps, C, lane4, one, gmin);
-                            ForR<VAR, 0>::run((double)(unsigned)rb.x, rb.y, rps, C, lane4, one, gmin);
-                            ForR<VAR, 0>::run((double)(unsigned)rb.z, rb.w, rps, C, lane4, one, gmin);
+                            ForR<0, IMM>::run((double)(unsigned)ra.x, ra.y, rps, C, lane4, sbase, gmin);
+                            ForR<0, IMM>::run((double)(unsigned)ra.z, ra.w, rps, C, lane4, sbase, gmin);
+                            ForR<0, IMM>::run((double)(unsigned)rb.x, rb.y, rps, C, lane4, sbase, gmin);
+                            ForR<0, IMM>::run((double)(unsigned)rb.z, rb.w, rps, C, lane4, sbase, gmin);
                         }
                     } else {
                         const int2 *st2 = reinterpret_cast<const int2 *>(stage);
 #pragma unroll 1
                         for (int s = 0; s < gc; ++s) {
                             const int2 rc = st2[s];
-                            ForR<VAR, 0>::run((double)(unsigned)rc.x, rc.y, rps, C, lane4, one, gmin);
+                            ForR<0, IMM>::run((double)(unsigned)rc.x, rc.y, rps, C, lane4, sbase, gmin);
                         }
                     }
                 }
@@ -349,7 +269,8 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     for (int r = 0; r < LP_R; ++r) {
                         if (gmin[r] >= D || !valid[r]) continue;
                         const double per = a.periods[p0 + r * 32 + lane];
-#pragma unroll 1
+                        if (a.stats) atomicAdd(a.stats + 1, 1ull);
+#pragma unroll 4
                         for (int s = 0; s < cnt; ++s) {
                             const int2 rc = __ldg(src + s);
                             double m = __fma_rd((double)(unsigned)rc.x, rps[r], C[r]);
@@ -357,8 +278,8 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                                 int kf = __double2hiint(m) & (LP_ROWS - 1);
                                 int ke = exact_bin(us[s], per, LP_ROWS);
                                 if (ke != kf) {
-                                    hist_update<VAR>(H, r, kf, lane, rc.y, -1);
-                                    if (ke >= 0) hist_update<VAR>(H, r, ke, lane, rc.y, +1);
+                                    hist_update(H, r, kf, lane, rc.y, -1);
+                                    if (ke >= 0) hist_update(H, r, ke, lane, rc.y, +1);
                                 }
                             }
                         }
@@ -367,6 +288,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
             }
         } else {
             // exact path: a period far outside the fast range or a tile spanning a huge gap
+            if (tid == 0 && a.stats) atomicAdd(a.stats + 0, 1ull);
             double per[LP_R];
 #pragma unroll
             for (int r = 0; r < LP_R; ++r)
@@ -388,7 +310,7 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                     for (int r = 0; r < LP_R; ++r) {
                         if (valid[r]) {
                             int ke = exact_bin(ui, per[r], LP_ROWS);
-                            if (ke >= 0) hist_update<VAR>(H, r, ke, lane, qi, +1);
+                            if (ke >= 0) hist_update(H, r, ke, lane, qi, +1);
                         }
                     }
                 }
@@ -397,29 +319,26 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
         __syncthreads();   // A: every update of this item is in H
 
         // ---- epilogue.  Lane l reads only its own columns: conflict-free, no cross-lane
-        // reduction.  Bin b = rows b*M .. b*M + M-1; a warp takes octets of bins (one
-        // 32-byte sector per output array) for all R period slots.
+        // reduction.  Bin b = rows b*M .. b*M + M-1; warp group g = warp / LP_WPR takes period
+        // slot r = g, its LP_WPR warps split the octets of bins (one 32-byte sector per output
+        // array and lane).
         const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
         const int octs = nb >> 3;
-        if constexpr (!V::PACKED) {
+        const int r = warp / LP_WPR, wr = warp - r * LP_WPR;
+        const long long j = p0 + r * 32 + lane;
+        const bool live = j < a.nperiods;
+        bool ok = false;
+#pragma unroll
+        for (int rr = 0; rr < LP_R; ++rr)
+            if (rr == r) ok = live && valid[rr];
+        unsigned *Hr = H + r * (LP_ROWS * 64) + lane;
         {
             // sweep 1: sums and counts out; bin mean m (of the centred flux) back into the
             // bin's first row as an fp64 {lo, hi} (NaN = empty); one-pass moments about the
-            // curve mean (exactly zero for a flat profile).  Warp group g = warp / WPR takes
-            // period slot r = g, its WPR warps split the octets of bins.
-            constexpr int WPR = LP_WARPS / LP_R;
-            static_assert(LP_WARPS % LP_R == 0, "warps per period slot");
-            const int r = warp / WPR, wr = warp - r * WPR;
+            // curve mean (exactly zero for a flat profile).
             double s1 = 0.0, s2 = 0.0;
             int kk = 0;
-            const long long j = p0 + r * 32 + lane;
-            const bool live = j < a.nperiods;
-            bool ok = false;
-#pragma unroll
-            for (int rr = 0; rr < LP_R; ++rr)
-                if (rr == r) ok = live && valid[rr];
-            unsigned *Hr = H + r * (LP_ROWS * 64) + lane;
-            for (int oct = wr; oct < octs; oct += WPR) {
+            for (int oct = wr; oct < octs; oct += LP_WPR) {
                 float fs[8];
                 unsigned fc[8];
 #pragma unroll
@@ -432,6 +351,10 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                         c += h0[jj * 64 + 32];
                         h0[jj * 64] = 0u;
                         h0[jj * 64 + 32] = 0u;
+                    }
+                    if (e == 0 && oct == 0) {       // the samples at u == 0 (CurveMeta::n_zero)
+                        S += cm.q_zero;
+                        c += (unsigned)cm.n_zero;
                     }
                     if (!ok) {
                         S = 0;
@@ -458,83 +381,24 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 }
                 if (live) {
                     const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
-                    if (a.out_sum) {
-                        float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
-                        o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
-                        o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
-                    }
-                    if (a.out_count) {
-                        uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
-                        o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
-                        o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
-                    }
-                }
-            }
-            if (want_norm) {
-                ps1[wr * LP_GROUP + r * 32 + lane] = s1;
-                ps2[wr * LP_GROUP + r * 32 + lane] = s2;
-                pkk[wr * LP_GROUP + r * 32 + lane] = kk;
-            }
-        }
-        } else {
-        {
-            // packed variants, sweep 1: sums and counts out; one-pass moments.  Count words are
-            // shared by two rows, so the counts are cleared
-            // after the last sweep; the sums are cleared here if this is the only sweep.
-            // Warp group g = warp / WPR takes period slot r = g.
-            constexpr int WPR = LP_WARPS / LP_R;
-            static_assert(LP_WARPS % LP_R == 0, "warps per period slot");
-            const int r = warp / WPR, wr = warp - r * WPR;
-            double s1 = 0.0, s2 = 0.0;
-            int kk = 0;
-            const long long j = p0 + r * 32 + lane;
-            const bool live = j < a.nperiods;
-            bool ok = false;
-#pragma unroll
-            for (int rr = 0; rr < LP_R; ++rr)
-                if (rr == r) ok = live && valid[rr];
-            for (int oct = wr; oct < octs; oct += WPR) {
-                float fs[8];
-                unsigned fc[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int row0 = (oct * 8 + e) * M;
-                    int S;
-                    unsigned c;
-                    read_bin<VAR>(H, r, row0, M, lane, S, c);
-                    for (int jj = 0; jj < M; ++jj) H[sum_word<VAR>(r, row0 + jj, lane)] = 0u;
-                    if (!ok) {
-                        S = 0;
-                        c = 0;
-                    }
-                    const double sq = __dmul_rn((double)S, inv_scale);
-                    fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
-                    fc[e] = c;
-                    if (want_norm) {
-                        // deviation of the bin mean from the curve mean, kept as fp32 in the
-                        // bin's (cleared) sum word for sweep 2: NaN = empty bin
-                        float df = __int_as_float(0x7fc00000);
-                        if (c > 0) {
-                            const double d = __dsub_rn(div_by_count(sq, c), pivot);
-                            s1 += d;
-                            s2 += __dmul_rn(d, d);
-                            kk += 1;
-                            df = (float)d;
+                    if (vec) {
+                        if (a.out_sum) {
+                            float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
+                            o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
+                            o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
                         }
-                        H[sum_word<VAR>(r, row0, lane)] = __float_as_uint(df);
-                    }
-                }
-                if (live) {
-                    const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
-                    if (a.out_sum) {
-                        float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
-                        o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
-                        o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
-                    }
-                    if (a.out_count) {
-                        uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
-                        o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
-                        o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
+                        if (a.out_count) {
+                            uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
+                            o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
+                            o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
+                        }
+                    } else {
+                        // outputs that are only 4-byte aligned: scalar stores
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            if (a.out_sum) a.out_sum[off + e] = fs[e];
+                            if (a.out_count) a.out_count[off + e] = fc[e];
+                        }
                     }
                 }
             }
@@ -543,15 +407,13 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 ps2[wr * LP_GROUP + r * 32 + lane] = s2;
                 pkk[wr * LP_GROUP + r * 32 + lane] = kk;
             }
-        }
         }
         if (want_norm) {
             __syncthreads();
             if (warp < LP_R) {
                 double s1 = 0.0, s2 = 0.0;
                 int kk = 0;
-                constexpr int NPART = LP_WARPS / LP_R;
-                for (int w = 0; w < NPART; ++w) {          // fixed order: deterministic
+                for (int w = 0; w < LP_WPR; ++w) {          // fixed order: deterministic
                     s1 += ps1[w * LP_GROUP + warp * 32 + lane];
                     s2 += ps2[w * LP_GROUP + warp * 32 + lane];
                     kk += pkk[w * LP_GROUP + warp * 32 + lane];
@@ -569,148 +431,68 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems, unsigned *probe)
                 st_kk[warp * 32 + lane] = kk;
             }
             __syncthreads();
-            if constexpr (!V::PACKED) {
             // sweep 2: normalised profile out, rows cleared (same split as sweep 1)
-            {
-                constexpr int WPR = LP_WARPS / LP_R;
-                const int r = warp / WPR, wr = warp - r * WPR;
-                const long long j = p0 + r * 32 + lane;
-                const bool live = j < a.nperiods;
-                bool okr = false;
+            const double mu = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
+            const double base_o = (ok && st_kk[r * 32 + lane] > 0) ? __dadd_rn(mu, center) : 0.0;
+            for (int oct = wr; oct < octs; oct += LP_WPR) {
+                float fn[8];
 #pragma unroll
-                for (int rr = 0; rr < LP_R; ++rr)
-                    if (rr == r) okr = valid[rr];
-                const double mu = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
-                const double base_o = (live && okr && st_kk[r * 32 + lane] > 0) ? __dadd_rn(mu, center) : 0.0;
-                unsigned *Hr = H + r * (LP_ROWS * 64) + lane;
-                for (int oct = wr; oct < octs; oct += WPR) {
-                    float fn[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        unsigned *h0 = Hr + (oct * 8 + e) * M * 64;
-                        const double m = __hiloint2double((int)h0[32], (int)h0[0]);
-                        h0[0] = 0u;
-                        h0[32] = 0u;
-                        double o = base_o;
-                        if (m == m && isd > 0.0) o = __dadd_rn(o, __dmul_rn(__dsub_rn(m, mu), isd));
-                        fn[e] = (float)o;
-                    }
-                    if (live) {
-                        float4 *o4 = reinterpret_cast<float4 *>(
-                            a.out_norm + ((curve * a.nperiods + j) * nb) + oct * 8);
+                for (int e = 0; e < 8; ++e) {
+                    unsigned *h0 = Hr + (oct * 8 + e) * M * 64;
+                    const double m = __hiloint2double((int)h0[32], (int)h0[0]);
+                    h0[0] = 0u;
+                    h0[32] = 0u;
+                    double o = base_o;
+                    if (m == m && isd > 0.0) o = __dadd_rn(o, __dmul_rn(__dsub_rn(m, mu), isd));
+                    fn[e] = (float)o;
+                }
+                if (live) {
+                    float *on = a.out_norm + ((curve * a.nperiods + j) * nb) + oct * 8;
+                    if (vec) {
+                        float4 *o4 = reinterpret_cast<float4 *>(on);
                         o4[0] = make_float4(fn[0], fn[1], fn[2], fn[3]);
                         o4[1] = make_float4(fn[4], fn[5], fn[6], fn[7]);
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) on[e] = fn[e];
                     }
                 }
             }
-            } else {
-            // packed variants, sweep 2: normalised profile from the fp32 deviations sweep 1
-            // left in the sum words (|d| is a few profile sigmas, so fp32 keeps (d - dm) / s to
-            // ~1e-6), sum words cleared (same split as sweep 1)
-            {
-                constexpr int WPR = LP_WARPS / LP_R;
-                const int r = warp / WPR, wr = warp - r * WPR;
-                const long long j = p0 + r * 32 + lane;
-                const bool live = j < a.nperiods;
-                bool okr = false;
-#pragma unroll
-                for (int rr = 0; rr < LP_R; ++rr)
-                    if (rr == r) okr = valid[rr];
-                const double mu = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
-                const double dm = __dsub_rn(mu, pivot);
-                const double base_o = (live && okr && st_kk[r * 32 + lane] > 0) ? __dadd_rn(mu, center) : 0.0;
-                for (int oct = wr; oct < octs; oct += WPR) {
-                    float fn[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        const int i0 = sum_word<VAR>(r, (oct * 8 + e) * M, lane);
-                        const float df = __uint_as_float(H[i0]);
-                        H[i0] = 0u;
-                        double o = base_o;
-                        if (okr && df == df && isd > 0.0)
-                            o = __dadd_rn(o, __dmul_rn(__dsub_rn((double)df, dm), isd));
-                        fn[e] = (float)o;
-                    }
-                    if (live) {
-                        float4 *o4 = reinterpret_cast<float4 *>(
-                            a.out_norm + ((curve * a.nperiods + j) * nb) + oct * 8);
-                        o4[0] = make_float4(fn[0], fn[1], fn[2], fn[3]);
-                        o4[1] = make_float4(fn[4], fn[5], fn[6], fn[7]);
-                    }
-                }
-            }
-            }
-        }
-        if constexpr (V::PACKED) {
-            // every row has been read: clear the packed counts
-            __syncthreads();
-            for (int i = tid; i < (LP_HIST_BYTES - LP_CNT1_OFF) / 4; i += LP_THREADS)
-                H[LP_CNT1_OFF / 4 + i] = 0u;
         }
         if (tid == 0) *ctr = 0;
         __syncthreads();   // B: H is zero again, tile counter reset
     }
 }
 
+__global__ void __launch_bounds__(LP_THREADS, 1)
+fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems)
+{
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(smem);
+    if (sbase == LP_WINDOW_BASE)
+        fold_lp_body<true>(a, ngroups, nitems, smem, sbase);
+    else
+        fold_lp_body<false>(a, ngroups, nitems, smem, sbase);
+}
+
 }  // namespace
 
-bool fold_lp_handles(int nbins)
+bool fold_lp_handles(int nbins) { return nbins == 32 || nbins == 64 || nbins == 128 || nbins == 256; }
+
+cudaError_t fold_lp_init_device()
 {
-    return nbins == 32 || nbins == 64 || nbins == 128 || nbins == 256 || nbins == 512 ||
-           nbins == 1024;
+    return cudaFuncSetAttribute(fold_lp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                LP_SMEM_BYTES);
 }
 
-int fold_lp_rows(int nbins) { return nbins <= 256 ? 256 : 1024; }
-
-template <int VAR>
-static cudaError_t launch_lp_var(FoldArgs a, cudaStream_t st)
+cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st, int sms)
 {
-    static int state = 0;   // 0 = not initialised, 1 = ready, -1 = shared-memory base differs
-    static std::mutex init_mutex;
-    auto kern = fold_lp_kernel<VAR>;
-    std::unique_lock<std::mutex> lock(init_mutex);
-    if (state == 0) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             LP_SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        unsigned *d = nullptr, h = 0;
-        e = cudaMalloc(reinterpret_cast<void **>(&d), sizeof(unsigned));
-        if (e != cudaSuccess) return e;
-        kern<<<1, LpV<VAR>::THREADS, LP_SMEM_BYTES, st>>>(a, 0, 0, d);
-        e = cudaMemcpyAsync(&h, d, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-        cudaFree(d);
-        if (e != cudaSuccess) return e;
-        state = (h == LP_SMEM_BASE) ? 1 : -1;
-    }
-    const int ready = state;
-    lock.unlock();
-    if (ready < 0) return cudaErrorInvalidConfiguration;   // never seen; reported, not worked around
-    constexpr int GROUP = 32 * LpV<VAR>::R;
-    const long long ngroups = (a.nperiods + GROUP - 1) / GROUP;
+    const long long ngroups = (a.nperiods + LP_GROUP - 1) / LP_GROUP;
     const long long nitems = ngroups * a.ncurves;
-    const long long grid = nitems < num_sms() ? nitems : num_sms();
-    kern<<<(unsigned)grid, LpV<VAR>::THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems, nullptr);
+    const long long grid = nitems < sms ? nitems : sms;
+    fold_lp_kernel<<<(unsigned)grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems);
+    note_launch();
     return cudaGetLastError();
-}
-
-cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st)
-{
-    // cudaErrorInvalidConfiguration from launch_lp_var = the shared-memory window does not start
-    // where the kernels' immediates assume (never seen): the exact generic kernel takes over
-    if (a.nbins <= 256) {
-        cudaError_t e = launch_lp_var<0>(a, st);
-        return (e == cudaErrorInvalidConfiguration) ? launch_fold_generic(a, st) : e;
-    }
-    // packed counts: curves of up to 65,535 valid samples here, longer ones in the generic kernel
-    FoldArgs b = a;
-    b.n_max = LP_PACKED_MAX_N;
-    cudaError_t e = launch_lp_var<1>(b, st);
-    if (e == cudaErrorInvalidConfiguration) return launch_fold_generic(a, st);
-    if (e != cudaSuccess) return e;
-    b = a;
-    b.n_min = LP_PACKED_MAX_N + 1;
-    return launch_fold_generic(b, st);
 }
 
 }  // namespace gpfc

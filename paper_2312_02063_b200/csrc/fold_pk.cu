@@ -1,0 +1,711 @@
+// fold_pk_kernel: the fold at 1024 / 2048 / 4096 rows (nbins 512 ... 4096), with the paper's
+// equal-count merge optionally fused into the epilogue (PAPER.md:105, :111 steps 1-5, Fig. 4;
+// noise normalisation :63).  DESIGN.md 6.2 has the derivation; in short:
+//
+// * One persistent CTA per SM, 24 warps.  A work item is (curve, group of PL consecutive trial
+//   periods), PL = 32768 / ROWS (32, 16, 8).  The 32 lanes of EVERY warp are PL periods x SL
+//   sample slots (SL = 32 / PL = 1, 2, 4): lane (slot, p) folds the samples of its slot at
+//   period p0 + p.  The warps split the curve's samples in anchor tiles.
+// * Histogram in shared memory: sums [row][PL] int32 (128 KB) and PACKED counts
+//   [row mod ROWS/2][PL] (64 KB): the low half-word counts rows k and k + ROWS/2 together, the
+//   high half-word counts row k + ROWS/2 alone.  The bank of a word is (row mod SL) * PL + p:
+//   one conflict-free wavefront per warp-wide atomic when SL = 1; for SL > 1 two slots collide
+//   when their rows agree mod SL (hardware replays, correctness is not affected).
+//   A half-word cannot overflow while at most 65,535 samples have been added, so the counts
+//   are flushed to a 32-bit side array in global memory (one per CTA, L2-resident) every
+//   65,408 samples: curves of any length stay on this kernel (the paper's Kepler curves have
+//   up to 70,000 epochs).
+// * Phase math, guard band and exact re-check: as in fold_lp.cu (one DFMA.RM per point-period,
+//   m = RD(v rp + C), row = bits of the high word, fraction = the low word; a tile whose
+//   smallest fraction is inside the guard band is re-checked against the exact formula).
+// * Epilogue, one of
+//   (1) bins: sums / counts (/ normalised profile) of nbins = ROWS >> k bins, written per lane;
+//   (2) merge: the nbins intermediary bins are merged left to right into nb2 bins of equal
+//       count (boundary bins split pro rata, R18) straight from the exact integer
+//       sums in shared memory -- the intermediary profile never reaches HBM -- then the mean
+//       and the noise-normalised profile of the nb2 bins are written.
+#include "common.cuh"
+
+namespace gpfc {
+
+namespace {
+
+constexpr int PK_THREADS = 768;
+constexpr int PK_WARPS = PK_THREADS / 32;
+constexpr int PK_GRAN = 64;                       // samples per staging granule
+constexpr int PK_CNT_OFF = 131072;                // byte offset of the packed counts
+constexpr int PK_HIST_BYTES = 196608;
+constexpr int PK_HIST_WORDS = PK_HIST_BYTES / 4;
+constexpr int PK_CELLS = 32768;                   // ROWS * PL, every variant
+constexpr int PK_SCR_OFF = PK_HIST_BYTES;         // scratch: staging | statistics partials | merge
+constexpr int PK_SCR_BYTES = 28672;
+constexpr int PK_CTR_OFF = PK_SCR_OFF + PK_SCR_BYTES;
+constexpr int PK_SMEM_BYTES = PK_CTR_OFF + 16;
+constexpr int PK_FLUSH_TILES = 511;               // 65,408 samples between count flushes
+constexpr int PK_NSEG = 16;                       // row segments of the merge scan
+// scratch, fold phase: int2 stage[PK_WARPS][PK_GRAN]                       12,288 B
+// scratch, bins epilogue: double ps1, ps2 [PK_WARPS][32]; int pkk [PK_WARPS][32];
+//                         double mu[32], isd[32]; int kk[32]                16,000 B
+constexpr int PK_PS1_OFF = PK_SCR_OFF;
+constexpr int PK_PS2_OFF = PK_PS1_OFF + PK_WARPS * 32 * 8;
+constexpr int PK_PKK_OFF = PK_PS2_OFF + PK_WARPS * 32 * 8;
+constexpr int PK_MU_OFF = PK_PKK_OFF + PK_WARPS * 32 * 4;
+constexpr int PK_ISD_OFF = PK_MU_OFF + 32 * 8;
+constexpr int PK_KK_OFF = PK_ISD_OFF + 32 * 8;
+// scratch, merge epilogue: unsigned segc[PK_NSEG][PL]; int segq[PK_NSEG][PL] (4 KB at most),
+//                          unsigned ntot[PL]; double scum[PL][nb2 + 1]      <= 24,448 B
+constexpr int PK_SEGC_OFF = PK_SCR_OFF;
+constexpr int PK_SEGQ_OFF = PK_SEGC_OFF + PK_NSEG * 32 * 4;
+constexpr int PK_NTOT_OFF = PK_SEGQ_OFF + PK_NSEG * 32 * 4;      // unsigned ntot[32]
+constexpr int PK_SCUM_OFF = PK_NTOT_OFF + 32 * 4;
+constexpr int PK_SCUM_BYTES = PK_SCR_OFF + PK_SCR_BYTES - PK_SCUM_OFF;
+static_assert(PK_KK_OFF + 32 * 4 <= PK_SCR_OFF + PK_SCR_BYTES, "bins-epilogue scratch");
+static_assert(PK_WARPS * PK_GRAN * 8 <= PK_SCR_BYTES, "staging scratch");
+static_assert(PK_SMEM_BYTES <= 227 * 1024, "shared memory budget");
+static_assert(GPFC_TILE == 2 * PK_GRAN, "half-tile work units are one staging granule");
+
+template <int ROWLOG>
+struct PkV {
+    static constexpr int ROWS = 1 << ROWLOG, HALF = ROWS / 2;
+    static constexpr int PLOG = 15 - ROWLOG, PL = 1 << PLOG;      // periods per work item
+    static constexpr int SLOG = 5 - PLOG, SL = 1 << SLOG;         // sample slots per warp
+    static constexpr int KSH = PLOG + 2;                          // log2 of the row stride in bytes
+    static constexpr unsigned SMASK = 0x1ffffu & ~((1u << KSH) - 1u);
+    static constexpr unsigned CMASK = 0x0ffffu & ~((1u << KSH) - 1u);
+};
+
+// shared-memory reduction with an immediate offset (ATOMS.ADD [R + UR + imm]: `addr` already
+// holds the shared-window address of the histogram, which ptxas keeps in a uniform register)
+template <int IMM>
+__device__ __forceinline__ void pk_red_add(unsigned addr, int v)
+{
+    asm volatile("red.shared.add.u32 [%0+%2], %1;" ::"r"(addr), "r"(v), "n"(IMM) : "memory");
+}
+
+// a value the compiler cannot see through, so that (x & mask) | p4 stays ONE LOP3
+__device__ __forceinline__ unsigned pk_opaque(unsigned x)
+{
+    unsigned y;
+    asm volatile("mov.u32 %0, %1;" : "=r"(y) : "r"(x));
+    return y;
+}
+
+// Shared-window address of dynamic shared memory on sm_100a (the first KB of the window is the
+// driver's): with this value the histogram offsets are instruction immediates.  The kernel
+// compares it with the real address and takes the register-base code path if they differ
+// (two more integer adds per point-period, same results), so nothing depends on it.
+constexpr unsigned PK_WINDOW_BASE = 0x400;
+
+// one point-period: row from the DFMA, two shared-memory atomics
+template <int ROWLOG, bool IMM>
+__device__ __forceinline__ void pk_update(double v, int q, double rps, double C, unsigned p4,
+                                          unsigned one, unsigned sbase, unsigned &gmin)
+{
+    using V = PkV<ROWLOG>;
+    const double m = __fma_rd(v, rps, C);
+    const unsigned lo = (unsigned)__double2loint(m), hi = (unsigned)__double2hiint(m);
+    gmin = min(gmin, lo);
+    const unsigned tt = hi << V::KSH;                      // row * (4 PL) (+ junk above bit 16)
+    const unsigned saddr = (tt & V::SMASK) | p4;           // row * 4 PL + p * 4
+    const unsigned caddr = (tt & V::CMASK) | p4;           // (row mod HALF) * 4 PL + p * 4
+    const unsigned val = (tt & 0x10000u) | one;            // 1 + ((row >= HALF) << 16)
+    if (IMM) {
+        pk_red_add<(int)PK_WINDOW_BASE>(saddr, q);
+        pk_red_add<(int)PK_WINDOW_BASE + PK_CNT_OFF>(caddr, (int)val);
+    } else {
+        pk_red_add<0>(saddr + sbase, q);
+        pk_red_add<PK_CNT_OFF>(caddr + sbase, (int)val);
+    }
+}
+
+// slow-path update of one sample: move = +1 adds it to `row`, -1 removes it
+template <int ROWLOG>
+__device__ __forceinline__ void pk_hist_update(unsigned *H, int row, int p, int q, int move)
+{
+    using V = PkV<ROWLOG>;
+    atomicAdd(&H[row * V::PL + p], (unsigned)(move * q));
+    atomicAdd(&H[PK_CNT_OFF / 4 + (row & (V::HALF - 1)) * V::PL + p],
+              (unsigned)move * (1u + ((unsigned)(row >> (ROWLOG - 1)) << 16)));
+}
+
+// count of (row, p): packed half-words in shared memory + the flushed part, if any
+template <int ROWLOG>
+__device__ __forceinline__ unsigned pk_count(const unsigned *H, const unsigned *side, int row, int p)
+{
+    using V = PkV<ROWLOG>;
+    const unsigned w = H[PK_CNT_OFF / 4 + (row & (V::HALF - 1)) * V::PL + p];
+    unsigned c = (row >> (ROWLOG - 1)) ? (w >> 16) : ((w & 0xffffu) - (w >> 16));
+    if (side) c += __ldcg(side + row * V::PL + p);
+    return c;
+}
+
+// sq / c for a count c in [1, 2^32): reciprocal from an fp32 seed + two Newton steps, then
+// one residual correction.  Exact whenever the quotient is representable, within 1 ulp
+// otherwise (same routine as fold_lp.cu).
+__device__ __forceinline__ double pk_div_by_count(double sq, unsigned c)
+{
+    const double cd = (double)c;
+    double r = (double)__frcp_rn((float)c);
+    r = __fma_rn(__fma_rn(-cd, r, 1.0), r, r);
+    r = __fma_rn(__fma_rn(-cd, r, 1.0), r, r);
+    const double q0 = __dmul_rn(sq, r);
+    return __fma_rn(__fma_rn(-q0, cd, sq), r, q0);
+}
+
+template <int ROWLOG, bool IMM>
+__device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroups, long long nitems,
+                                             unsigned char *smem, unsigned sbase)
+{
+    using V = PkV<ROWLOG>;
+    constexpr int ROWS = V::ROWS, HALF = V::HALF, PL = V::PL, PLOG = V::PLOG, SL = V::SL;
+    unsigned *H = reinterpret_cast<unsigned *>(smem);
+    int *ctr = reinterpret_cast<int *>(smem + PK_CTR_OFF);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int p = lane & (PL - 1), slot = lane >> PLOG;
+    const unsigned p4 = pk_opaque((unsigned)p << 2);
+    const unsigned one = pk_opaque((unsigned)(a.nbins > 0));   // 1, not foldable
+    int4 *stage4 = reinterpret_cast<int4 *>(smem + PK_SCR_OFF) + warp * (PK_GRAN / 2);
+    for (int i = tid; i < PK_HIST_WORDS; i += PK_THREADS) H[i] = 0u;
+    if (tid == 0) *ctr = 0;
+    __syncthreads();
+
+    const int nb = a.nbins;                               // power of two, ROWS / 2 <= nb <= ROWS
+    const int mshift = ROWLOG - (31 - __clz(nb));         // rows merged per bin = 1 << mshift
+    const int M = 1 << mshift;
+    const double M2 = 6755399441055744.0 * (double)ROWS;  // 1.5 * 2^(52 + ROWLOG): ulp = ROWS
+    unsigned *side = a.side ? a.side + (size_t)blockIdx.x * PK_CELLS : nullptr;
+
+    for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const long long curve = item / ngroups;
+        const long long p0 = (item - curve * ngroups) * PL;
+        const CurveMeta cm = a.meta[curve];
+        const int n = cm.n_valid;
+        const int ntiles = (n + GPFC_TILE - 1) / GPFC_TILE;
+
+        // this lane's period
+        const long long j = p0 + p;
+        const bool live = j < a.nperiods;
+        const double x = live ? a.rp[j] : CUDART_NAN;
+        const bool valid = (x == x);
+        const double rp = valid ? x : (double)ROWS;       // dummy: its column is never written out
+        double rpmax = valid ? x : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) rpmax = fmax(rpmax, __shfl_xor_sync(0xffffffffu, rpmax, o));
+
+        // guard band, units of 2^-32 row; see fold_lp.cu
+        const double U = fmax(fabs(cm.umin), fabs(cm.umax));
+        const double ebase = 4.0 * U * rpmax * (1.0 / 2097152.0) + 1.0;
+        const double eq_max = fmax(2.0 * cm.span_max, 1.0 / 256.0) * rpmax;
+        const bool fast = (2.0 * (ebase + eq_max) + 2.0 <= 1048576.0) &&
+                          (cm.span_max * rpmax + 2.0 * ROWS < 1048576.0);
+        if (!fast && tid == 0 && a.stats) atomicAdd(a.stats + 0, 1ull);
+        const double per_exact = (valid && !fast) ? a.periods[j] : 1.0;
+
+        const int nseg = (ntiles + PK_FLUSH_TILES - 1) / PK_FLUSH_TILES;
+        for (int seg = 0; seg < nseg; ++seg) {
+            const int t_lo = seg * PK_FLUSH_TILES;
+            const int t_n = min(ntiles - t_lo, PK_FLUSH_TILES);
+            if (fast) {
+                // work units: whole anchor tiles first, the last 2 * PK_WARPS tiles in halves
+                const int nfull = max(0, t_n - 2 * PK_WARPS);
+                const int nunits = nfull + 2 * (t_n - nfull);
+                for (;;) {
+                    int u = 0;
+                    if (lane == 0) u = atomicAdd(ctr, 1);
+                    u = __shfl_sync(0xffffffffu, u, 0);
+                    if (u >= nunits) break;
+                    const int t = t_lo + ((u < nfull) ? u : nfull + ((u - nfull) >> 1));
+                    const int half = (u < nfull) ? 0 : ((u - nfull) & 1);
+                    const int base = t * GPFC_TILE + half * PK_GRAN;
+                    const int cnt = min((u < nfull) ? GPFC_TILE : PK_GRAN, n - base);
+                    if (cnt <= 0) continue;
+                    const TileInfo ti = a.tiles[cm.tile0 + t];
+                    const double need = 2.0 * (ebase + 0.5 * ti.inv_scale * rpmax * 4294967296.0) + 2.0;
+                    unsigned D = ((unsigned)need + 2u) & ~1u;
+                    if (D < 16u) D = 16u;
+                    const double K = 1048576.0 + (double)(D >> 1) * (1.0 / 4294967296.0);
+                    const double w = __fma_rd(ti.a, rp, M2);          // M2 + ROWS floor(a rp / ROWS)
+                    const double z = __dsub_rn(w, M2);
+                    const double c1 = __fma_rn(ti.a, rp, -z);         // (a rp) mod ROWS
+                    const double C = __dadd_rn(c1, K);
+                    const double rps = __dmul_rn(rp, ti.inv_scale);   // exact (power of two)
+                    const int2 *src = a.rec + cm.rec0 + base;         // 16-byte aligned
+                    const int4 *src4 = reinterpret_cast<const int4 *>(src);
+                    unsigned gmin = 0xffffffffu;
+                    int4 nx = make_int4(0, 0, 0, 0);
+                    if (2 * lane < cnt) nx = __ldg(src4 + lane);
+                    for (int g0 = 0; g0 < cnt; g0 += PK_GRAN) {
+                        const int gc = min(PK_GRAN, cnt - g0);
+                        __syncwarp();
+                        stage4[lane] = nx;
+                        __syncwarp();
+                        if (g0 + PK_GRAN + 2 * lane < cnt) nx = __ldg(src4 + (g0 + PK_GRAN) / 2 + lane);
+                        if (gc == PK_GRAN) {
+                            // slot s takes the sample pairs s, s + SL, s + 2 SL, ...
+#pragma unroll 1
+                            for (int g = 0; g < PK_GRAN / 2; g += 2 * SL) {
+                                const int4 ra = stage4[g + slot], rb = stage4[g + SL + slot];
+                                pk_update<ROWLOG, IMM>((double)(unsigned)ra.x, ra.y, rps, C, p4, one, sbase, gmin);
+                                pk_update<ROWLOG, IMM>((double)(unsigned)ra.z, ra.w, rps, C, p4, one, sbase, gmin);
+                                pk_update<ROWLOG, IMM>((double)(unsigned)rb.x, rb.y, rps, C, p4, one, sbase, gmin);
+                                pk_update<ROWLOG, IMM>((double)(unsigned)rb.z, rb.w, rps, C, p4, one, sbase, gmin);
+                            }
+                        } else {
+                            const int2 *st2 = reinterpret_cast<const int2 *>(stage4);
+#pragma unroll 1
+                            for (int s = slot; s < gc; s += SL) {
+                                const int2 rc = st2[s];
+                                pk_update<ROWLOG, IMM>((double)(unsigned)rc.x, rc.y, rps, C, p4, one, sbase, gmin);
+                            }
+                        }
+                    }
+                    if (__any_sync(0xffffffffu, gmin < D)) {
+                        // rare: a row coordinate sat within the guard band of an integer.  The
+                        // flagged lanes re-check THEIR samples (same enumeration as above)
+                        // against the exact formula and move the ones in the wrong row.
+                        if (gmin < D && valid) {
+                            const double per = a.periods[j];
+                            const double *us = a.u + cm.start + base;
+                            if (a.stats) atomicAdd(a.stats + 1, 1ull);
+                            for (int g0 = 0; g0 < cnt; g0 += PK_GRAN) {
+                                const int gc = min(PK_GRAN, cnt - g0);
+                                const int ns = (gc == PK_GRAN) ? PK_GRAN / SL : (gc - slot + SL - 1) / SL;
+#pragma unroll 4
+                                for (int i = 0; i < ns; ++i) {
+                                    // i-th sample of this slot in the granule
+                                    const int s = (gc == PK_GRAN) ? (((i >> 1) * SL + slot) * 2 + (i & 1))
+                                                                  : (slot + i * SL);
+                                    const int2 rc = __ldg(src + g0 + s);
+                                    const double m = __fma_rd((double)(unsigned)rc.x, rps, C);
+                                    if ((unsigned)__double2loint(m) < D) {
+                                        const int kf = __double2hiint(m) & (ROWS - 1);
+                                        const int ke = exact_bin(us[g0 + s], per, ROWS);
+                                        if (ke != kf) {
+                                            pk_hist_update<ROWLOG>(H, kf, p, rc.y, -1);
+                                            if (ke >= 0) pk_hist_update<ROWLOG>(H, ke, p, rc.y, +1);
+                                        }
+                                    }
+                                }
+                            }
+                        }
+                    }
+                }
+            } else {
+                // exact path: a period far outside the fast range or a tile spanning a huge gap
+                for (;;) {
+                    int t = 0;
+                    if (lane == 0) t = atomicAdd(ctr, 1);
+                    t = __shfl_sync(0xffffffffu, t, 0);
+                    if (t >= t_n) break;
+                    const int base = (t_lo + t) * GPFC_TILE;
+                    const int cnt = min(GPFC_TILE, n - base);
+                    const double *us = a.u + cm.start + base;
+                    const int *qs = a.q + cm.start + base;
+                    if (valid) {
+#pragma unroll 1
+                        for (int s = slot; s < cnt; s += SL) {
+                            const int ke = exact_bin(us[s], per_exact, ROWS);
+                            if (ke >= 0) pk_hist_update<ROWLOG>(H, ke, p, qs[s], +1);
+                        }
+                    }
+                }
+            }
+            __syncthreads();   // every update of this segment is in H
+            if (seg + 1 < nseg) {
+                // count flush: the packed half-words go to the 32-bit side array
+                for (int i = tid; i < HALF * PL; i += PK_THREADS) {
+                    const unsigned w = H[PK_CNT_OFF / 4 + i];
+                    const unsigned chi = w >> 16, clo = (w & 0xffffu) - chi;
+                    if (seg == 0) {
+                        side[i] = clo;
+                        side[i + HALF * PL] = chi;
+                    } else {
+                        side[i] += clo;
+                        side[i + HALF * PL] += chi;
+                    }
+                    H[PK_CNT_OFF / 4 + i] = 0u;
+                }
+                if (tid == 0) *ctr = 0;
+                __syncthreads();
+            }
+        }
+        const unsigned *sd = (nseg > 1) ? side : nullptr;
+        const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
+        const bool ok = live && valid;
+
+        if (a.nb2 == 0) {
+            // ---- epilogue (1): bins.  Lane (slot, p) takes the bins blk * 8 SL + e * SL + slot,
+            // e = 0..7, of period p: rows of different slots differ mod SL (conflict-free).
+            double *ps1 = reinterpret_cast<double *>(smem + PK_PS1_OFF);
+            double *ps2 = reinterpret_cast<double *>(smem + PK_PS2_OFF);
+            int *pkk = reinterpret_cast<int *>(smem + PK_PKK_OFF);
+            double *st_mu = reinterpret_cast<double *>(smem + PK_MU_OFF);
+            double *st_isd = reinterpret_cast<double *>(smem + PK_ISD_OFF);
+            int *st_kk = reinterpret_cast<int *>(smem + PK_KK_OFF);
+            const bool want_norm = a.out_norm != nullptr;
+            const int nblk = nb / (8 * SL);
+            const long long orow = (curve * a.nperiods + j) * nb;
+            double s1 = 0.0, s2 = 0.0;
+            int kk = 0;
+            for (int blk = warp; blk < nblk; blk += PK_WARPS) {
+                float fs[8];
+                unsigned fc[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int bin = blk * 8 * SL + e * SL + slot;
+                    int S = 0;
+                    unsigned c = 0;
+                    for (int jj = 0; jj < M; ++jj) {
+                        const int row = bin * M + jj;
+                        S += (int)H[row * PL + p];
+                        c += pk_count<ROWLOG>(H, sd, row, p);
+                        H[row * PL + p] = 0u;
+                    }
+                    if (e == 0 && bin == 0) {       // the samples at u == 0 (CurveMeta::n_zero)
+                        S += cm.q_zero;
+                        c += (unsigned)cm.n_zero;
+                    }
+                    if (!ok) {
+                        S = 0;
+                        c = 0;
+                    }
+                    const double sq = __dmul_rn((double)S, inv_scale);
+                    fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
+                    fc[e] = c;
+                    if (want_norm) {
+                        // deviation of the bin mean from the curve mean, kept as fp32 in the
+                        // bin's (cleared) sum word for sweep 2: NaN = empty bin
+                        float df = __int_as_float(0x7fc00000);
+                        if (c > 0) {
+                            const double d = __dsub_rn(pk_div_by_count(sq, c), pivot);
+                            s1 += d;
+                            s2 += __dmul_rn(d, d);
+                            kk += 1;
+                            df = (float)d;
+                        }
+                        H[bin * M * PL + p] = __float_as_uint(df);
+                    }
+                }
+                if (live) {
+                    const long long off = orow + blk * 8 * SL + slot;
+                    if (SL == 1 && a.vec_ok) {
+                        if (a.out_sum) {
+                            float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
+                            o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
+                            o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
+                        }
+                        if (a.out_count) {
+                            uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
+                            o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
+                            o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
+                        }
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            if (a.out_sum) a.out_sum[off + e * SL] = fs[e];
+                            if (a.out_count) a.out_count[off + e * SL] = fc[e];
+                        }
+                    }
+                }
+            }
+            if (want_norm) {
+                ps1[warp * 32 + lane] = s1;
+                ps2[warp * 32 + lane] = s2;
+                pkk[warp * 32 + lane] = kk;
+                __syncthreads();
+                if (tid < PL) {
+                    double t1 = 0.0, t2 = 0.0;
+                    int tk = 0;
+                    for (int w = 0; w < PK_WARPS; ++w)            // fixed order: deterministic
+                        for (int s = 0; s < SL; ++s) {
+                            t1 += ps1[w * 32 + s * PL + tid];
+                            t2 += ps2[w * 32 + s * PL + tid];
+                            tk += pkk[w * 32 + s * PL + tid];
+                        }
+                    double mu = 0.0, isd = 0.0;
+                    if (tk > 0) {
+                        const double dm = __ddiv_rn(t1, (double)tk);
+                        mu = __dadd_rn(pivot, dm);
+                        const double var = __dsub_rn(__ddiv_rn(t2, (double)tk), __dmul_rn(dm, dm));
+                        const double sdv = (var > 0.0) ? sqrt(var) : 0.0;
+                        if (tk >= 2 && sdv > 0.0) isd = __ddiv_rn(1.0, sdv);
+                    }
+                    st_mu[tid] = mu;
+                    st_isd[tid] = isd;
+                    st_kk[tid] = tk;
+                }
+                __syncthreads();
+                // sweep 2: normalised profile from the fp32 deviations (|d| is a few profile
+                // sigmas, so fp32 keeps (d - dm) / s to ~1e-6), sum words cleared
+                const double mu = st_mu[p], isd = st_isd[p];
+                const double dm = __dsub_rn(mu, pivot);
+                const double base_o = (ok && st_kk[p] > 0) ? __dadd_rn(mu, center) : 0.0;
+                for (int blk = warp; blk < nblk; blk += PK_WARPS) {
+                    float fn[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int i0 = (blk * 8 * SL + e * SL + slot) * M * PL + p;
+                        const float df = __uint_as_float(H[i0]);
+                        H[i0] = 0u;
+                        double o = base_o;
+                        if (ok && df == df && isd > 0.0)
+                            o = __dadd_rn(o, __dmul_rn(__dsub_rn((double)df, dm), isd));
+                        fn[e] = (float)o;
+                    }
+                    if (live) {
+                        const long long off = orow + blk * 8 * SL + slot;
+                        if (SL == 1 && a.vec_ok) {
+                            float4 *o4 = reinterpret_cast<float4 *>(a.out_norm + off);
+                            o4[0] = make_float4(fn[0], fn[1], fn[2], fn[3]);
+                            o4[1] = make_float4(fn[4], fn[5], fn[6], fn[7]);
+                        } else {
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) a.out_norm[off + e * SL] = fn[e];
+                        }
+                    }
+                }
+            }
+            // every row has been read: clear the packed counts
+            __syncthreads();
+            for (int i = tid; i < HALF * PL; i += PK_THREADS) H[PK_CNT_OFF / 4 + i] = 0u;
+        } else {
+            // ---- epilogue (2): equal-count merge of the nb = ROWS intermediary bins into nb2
+            // bins ("Fourthly", reading R18), per period p:
+            //   N = total count, per = N / nb2, target_b = per (b + 1) (= N for the last bin);
+            //   boundary b lies in the first row k with C(k) >= target_b (C = cumulative count),
+            //   Scum_b = S(k-1) + ((target_b - C(k-1)) / count_k) sum_k,
+            //   mean_b = (Scum_b - Scum_{b-1}) / per.
+            // The rows are scanned in PK_NSEG segments (one warp each, 64 steps of SL rows: the
+            // SL slots read SL consecutive rows, conflict-free); cumulative counts and integer
+            // sums are exact (|any partial sum of q| < 2^31 by the choice of the scale).
+            unsigned *segc = reinterpret_cast<unsigned *>(smem + PK_SEGC_OFF);
+            int *segq = reinterpret_cast<int *>(smem + PK_SEGQ_OFF);
+            unsigned *ntot_s = reinterpret_cast<unsigned *>(smem + PK_NTOT_OFF);
+            double *scum = reinterpret_cast<double *>(smem + PK_SCUM_OFF);
+            const int nb2 = a.nb2;
+            constexpr int RPS = ROWS / PK_NSEG;            // rows per segment
+            if (cm.n_zero > 0) {
+                // the samples at u == 0 (CurveMeta::n_zero, at most 255) belong to row 0
+                if (tid < PL) {
+                    H[tid] += (unsigned)cm.q_zero;
+                    H[PK_CNT_OFF / 4 + tid] += (unsigned)cm.n_zero;
+                }
+                __syncthreads();
+            }
+            constexpr int STEPS = RPS / SL;                // 64
+            if (warp < PK_NSEG) {
+                unsigned tc = 0;
+                int tq = 0;
+                const int r0 = warp * RPS + slot;
+#pragma unroll 4
+                for (int i = 0; i < STEPS; ++i) {
+                    const int row = r0 + i * SL;
+                    tc += pk_count<ROWLOG>(H, sd, row, p);
+                    tq += (int)H[row * PL + p];
+                }
+#pragma unroll
+                for (int o = PL; o < 32; o <<= 1) {
+                    tc += __shfl_xor_sync(0xffffffffu, tc, o);
+                    tq += __shfl_xor_sync(0xffffffffu, tq, o);
+                }
+                if (slot == 0) {
+                    segc[warp * PL + p] = tc;
+                    segq[warp * PL + p] = tq;
+                }
+            }
+            __syncthreads();
+            if (warp < PK_NSEG) {
+                unsigned cb = 0, ntot = 0;       // points before this segment, total
+                int qb = 0;                      // integer flux before this segment
+                for (int s = 0; s < PK_NSEG; ++s) {
+                    const unsigned c = segc[s * PL + p];
+                    if (s < warp) {
+                        cb += c;
+                        qb += segq[s * PL + p];
+                    }
+                    ntot += c;
+                }
+                if (!ok) ntot = 0;
+                const double total = (double)ntot;
+                const double per = __ddiv_rn(total, (double)nb2);
+                double *sc = scum + p * (nb2 + 1);
+                const bool act = ntot > 0u;      // per lane (period); the shuffles below are warp-wide
+                // next boundary not yet emitted, its target and thr = ceil(target):
+                // C >= target  <=>  C >= thr for an integer C
+                int b = nb2;
+                double target = 0.0;
+                unsigned thr = 0xffffffffu;
+                auto set_b = [&](int bb) {
+                    b = bb;
+                    if (b < nb2) {
+                        target = (b == nb2 - 1) ? total : __dmul_rn(per, (double)(b + 1));
+                        thr = (unsigned)ceil(target);
+                    } else {
+                        thr = 0xffffffffu;
+                    }
+                };
+                for (int i = 0; i < STEPS; ++i) {
+                    const int row = warp * RPS + i * SL + slot;
+                    const unsigned c = pk_count<ROWLOG>(H, sd, row, p);
+                    const int q = (int)H[row * PL + p];
+                    // inclusive prefix over the SL slots of this step (slot s = lanes s * PL + p)
+                    unsigned ci = c;
+                    int qi = q;
+#pragma unroll
+                    for (int o = 1; o < SL; o <<= 1) {
+                        const unsigned cu = __shfl_up_sync(0xffffffffu, ci, o * PL);
+                        const int qu = __shfl_up_sync(0xffffffffu, qi, o * PL);
+                        if (slot >= o) {
+                            ci += cu;
+                            qi += qu;
+                        }
+                    }
+                    const unsigned cbef = cb + ci - c, cinc = cb + ci;     // C(row - 1), C(row)
+                    const int qbef = qb + qi - q;
+                    cb += __shfl_sync(0xffffffffu, ci, (SL - 1) * PL + p);
+                    qb += __shfl_sync(0xffffffffu, qi, (SL - 1) * PL + p);
+                    if (!act) continue;
+                    if (i == 0) {
+                        // first boundary whose target lies beyond the points before this row
+                        int bb = (int)floor(__ddiv_rn((double)cbef, per)) - 1;
+                        if (bb < 0 || cbef == 0u) bb = 0;
+                        set_b(bb);
+                    }
+                    // boundaries reached by earlier rows (other slots, other segments)
+                    while (thr <= cbef) set_b(b + 1);
+                    const bool last = (row == ROWS - 1);
+                    if (b < nb2 && (last || thr <= cinc)) {
+                        const double ck = (double)c, cbd = (double)cbef;
+                        const double sbef = __dadd_rn(__dmul_rn((double)qbef, inv_scale),
+                                                      __dmul_rn(cbd, center));
+                        const double sk = __dadd_rn(__dmul_rn((double)q, inv_scale),
+                                                    __dmul_rn(ck, center));
+                        do {
+                            double frac = (c > 0u) ? __ddiv_rn(__dsub_rn(target, cbd), ck) : 0.0;
+                            frac = fmin(fmax(frac, 0.0), 1.0);
+                            sc[b + 1] = __dadd_rn(sbef, __dmul_rn(frac, sk));
+                            set_b(b + 1);
+                        } while (b < nb2 && (last || thr <= cinc));
+                    }
+                }
+                if (warp == 0 && slot == 0) {
+                    sc[0] = 0.0;
+                    ntot_s[p] = ntot;
+                }
+            }
+            __syncthreads();
+            // means, optional normalisation (mean kept, population std 1 over the nb2 bins):
+            // one warp per period, same arithmetic as merge.cu
+            for (int pp = warp; pp < PL; pp += PK_WARPS) {
+                const long long jj = p0 + pp;
+                if (jj >= a.nperiods) continue;
+                const unsigned ntot = ntot_s[pp];
+                const long long off = (curve * a.nperiods + jj) * nb2;
+                if (ntot == 0u) {
+                    for (int bb = lane; bb < nb2; bb += 32) {
+                        if (a.out_mean2) a.out_mean2[off + bb] = 0.f;
+                        if (a.out_norm2) a.out_norm2[off + bb] = 0.f;
+                    }
+                    continue;
+                }
+                const double per = __ddiv_rn((double)ntot, (double)nb2);
+                const double *sc = scum + pp * (nb2 + 1);
+                double acc = 0.0;
+                for (int bb = lane; bb < nb2; bb += 32) {
+                    const double m = __ddiv_rn(__dsub_rn(sc[bb + 1], sc[bb]), per);
+                    if (a.out_mean2) a.out_mean2[off + bb] = (float)m;
+                    acc += m;
+                }
+                if (a.out_norm2) {
+                    acc = warp_sum(acc);
+                    const double mu = __ddiv_rn(acc, (double)nb2);
+                    double vacc = 0.0;
+                    for (int bb = lane; bb < nb2; bb += 32) {
+                        const double d = __dsub_rn(__ddiv_rn(__dsub_rn(sc[bb + 1], sc[bb]), per), mu);
+                        vacc += __dmul_rn(d, d);
+                    }
+                    vacc = warp_sum(vacc);
+                    const double sdv = sqrt(__ddiv_rn(vacc, (double)nb2));
+                    const bool flat = (nb2 < 2) || !(sdv > 0.0);
+                    for (int bb = lane; bb < nb2; bb += 32) {
+                        const double m = __ddiv_rn(__dsub_rn(sc[bb + 1], sc[bb]), per);
+                        const double o = flat ? mu : __dadd_rn(mu, __ddiv_rn(__dsub_rn(m, mu), sdv));
+                        a.out_norm2[off + bb] = (float)o;
+                    }
+                }
+            }
+            __syncthreads();
+            // clear the whole histogram
+            uint4 *H4 = reinterpret_cast<uint4 *>(H);
+            for (int i = tid; i < PK_HIST_BYTES / 16; i += PK_THREADS) H4[i] = make_uint4(0u, 0u, 0u, 0u);
+        }
+        if (tid == 0) *ctr = 0;
+        __syncthreads();   // H is zero again, tile counter reset
+    }
+}
+
+template <int ROWLOG>
+__global__ void __launch_bounds__(PK_THREADS, 1)
+fold_pk_kernel(FoldArgs a, long long ngroups, long long nitems)
+{
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(smem);
+    if (sbase == PK_WINDOW_BASE)
+        fold_pk_body<ROWLOG, true>(a, ngroups, nitems, smem, sbase);
+    else
+        fold_pk_body<ROWLOG, false>(a, ngroups, nitems, smem, sbase);
+}
+
+template <int ROWLOG>
+cudaError_t pk_set_attr()
+{
+    return cudaFuncSetAttribute(fold_pk_kernel<ROWLOG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                PK_SMEM_BYTES);
+}
+
+template <int ROWLOG>
+cudaError_t pk_launch(const FoldArgs &a, cudaStream_t st, int sms)
+{
+    constexpr int PL = PkV<ROWLOG>::PL;
+    const long long ngroups = (a.nperiods + PL - 1) / PL;
+    const long long nitems = ngroups * a.ncurves;
+    const long long grid = nitems < sms ? nitems : sms;
+    fold_pk_kernel<ROWLOG><<<(unsigned)grid, PK_THREADS, PK_SMEM_BYTES, st>>>(a, ngroups, nitems);
+    note_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+bool fold_pk_handles(int nbins) { return nbins == 512 || nbins == 1024 || nbins == 2048 || nbins == 4096; }
+
+int fold_pk_rows(int nbins) { return nbins <= 1024 ? 1024 : nbins; }
+
+bool fold_pk_can_merge(int nbins, int nb2)
+{
+    if (!(nbins == 1024 || nbins == 2048 || nbins == 4096) || nb2 < 1) return false;
+    const int pl = 32768 / nbins;
+    return (size_t)pl * (size_t)(nb2 + 1) * 8 <= (size_t)PK_SCUM_BYTES;
+}
+
+size_t fold_pk_side_bytes(int sms) { return (size_t)sms * PK_CELLS * sizeof(unsigned); }
+
+long long fold_pk_flush_samples() { return (long long)PK_FLUSH_TILES * GPFC_TILE; }
+
+cudaError_t fold_pk_init_device()
+{
+    cudaError_t e = pk_set_attr<10>();
+    if (e == cudaSuccess) e = pk_set_attr<11>();
+    if (e == cudaSuccess) e = pk_set_attr<12>();
+    return e;
+}
+
+cudaError_t launch_fold_pk(const FoldArgs &a, cudaStream_t st, int sms)
+{
+    if (a.nbins <= 1024) return pk_launch<10>(a, st, sms);
+    if (a.nbins == 2048) return pk_launch<11>(a, st, sms);
+    return pk_launch<12>(a, st, sms);
+}
+
+}  // namespace gpfc

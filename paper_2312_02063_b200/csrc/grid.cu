@@ -38,6 +38,7 @@ cudaError_t launch_grid(double pmin, double pmax, long long nperiods, int mode_f
     if (nperiods <= 0) return cudaSuccess;
     unsigned blocks = (unsigned)((nperiods + 255) / 256);
     grid_kernel<<<blocks, 256, 0, st>>>(pmin, pmax, nperiods, mode_flags, out);
+    note_launch();
     return cudaGetLastError();
 }
 

@@ -181,6 +181,12 @@ merge_equal_count_kernel(const float *__restrict__ sum, const uint32_t *__restri
 
 }  // namespace
 
+cudaError_t merge_init_device()
+{
+    return cudaFuncSetAttribute(merge_equal_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                200 * 1024);
+}
+
 cudaError_t launch_merge(const float *sum, const uint32_t *count, long long nprofiles, int nb1,
                          int nb2, float *out_mean, float *out_norm, cudaStream_t st)
 {
@@ -192,13 +198,9 @@ cudaError_t launch_merge(const float *sum, const uint32_t *count, long long npro
     long long blocks = (nprofiles + warps - 1) / warps;
     if (blocks > 148LL * 16) blocks = 148LL * 16;
     size_t smem = (size_t)warps * per_warp;
-    if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(merge_equal_count_kernel,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-    }
     merge_equal_count_kernel<<<(unsigned)blocks, warps * 32, smem, st>>>(
         sum, count, nprofiles, nb1, nb2, out_mean, out_norm);
+    note_launch();
     return cudaGetLastError();
 }
 

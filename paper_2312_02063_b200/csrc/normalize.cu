@@ -66,6 +66,7 @@ cudaError_t launch_normalize(const float *sum, const uint32_t *count, long long 
     long long blocks = (nprofiles + wpb - 1) / wpb;
     if (blocks > 148LL * 32) blocks = 148LL * 32;
     normalize_kernel<<<(unsigned)blocks, NORM_THREADS, 0, st>>>(sum, count, nprofiles, nbins, out);
+    note_launch();
     return cudaGetLastError();
 }
 

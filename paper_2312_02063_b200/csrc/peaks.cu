@@ -143,7 +143,8 @@ __global__ void __launch_bounds__(768, 1) peak_loop_kernel(int nsamples, double 
         rec[threadIdx.x] = make_int4(threadIdx.x * 40503 + 17, (int)threadIdx.x - 30,
                                      threadIdx.x * 65599 + 3, 31 - (int)threadIdx.x);
     __syncthreads();
-    const unsigned lane4 = (unsigned)lane << 2;   // + 0x400 (shared-window base) in the immediates
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(peaks_smem);   // kept in a uniform register
+    const unsigned lane4 = (unsigned)lane << 2;
     double rp[3], C[3];
 #pragma unroll
     for (int r = 0; r < 3; ++r) {
@@ -163,11 +164,11 @@ __global__ void __launch_bounds__(768, 1) peak_loop_kernel(int nsamples, double 
             for (int r = 0; r < 3; ++r) {
                 double m = __fma_rd(v, rp[r], C[r]);
                 unsigned lo = (unsigned)__double2loint(m), hi = (unsigned)__double2hiint(m);
-                unsigned addr = __byte_perm(lane4, hi, 0x3240);
+                unsigned addr = __byte_perm(lane4, hi, 0x3240) + sbase;
                 gmin = min(gmin, lo);
-                if (r == 0) { pk_red_add<0x400>(addr, q[k]); pk_red_inc<0x400 + 128>(addr); }
-                if (r == 1) { pk_red_add<0x400 + 65536>(addr, q[k]); pk_red_inc<0x400 + 65536 + 128>(addr); }
-                if (r == 2) { pk_red_add<0x400 + 131072>(addr, q[k]); pk_red_inc<0x400 + 131072 + 128>(addr); }
+                if (r == 0) { pk_red_add<0>(addr, q[k]); pk_red_inc<128>(addr); }
+                if (r == 1) { pk_red_add<65536>(addr, q[k]); pk_red_inc<65536 + 128>(addr); }
+                if (r == 2) { pk_red_add<131072>(addr, q[k]); pk_red_inc<131072 + 128>(addr); }
             }
         }
     }

@@ -72,7 +72,7 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     // pass 1: L1 norm, sum, count, range of u over the valid samples
-    double a0 = 0.0, sm = 0.0, cnt = 0.0, umin = CUDART_INF, nmax = CUDART_INF;
+    double a0 = 0.0, sm = 0.0, cnt = 0.0, cnt0 = 0.0, umin = CUDART_INF, nmax = CUDART_INF;
     for (long long i = tid; i < n; i += PREP_THREADS) {
         double ti = t[i];
         float fi = f[i];
@@ -81,6 +81,7 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
             a0 += fabs((double)fi);
             sm += (double)fi;
             cnt += 1.0;
+            if (u == 0.0) cnt0 += 1.0;
             umin = fmin(umin, u);
             nmax = fmin(nmax, -u);
         }
@@ -88,6 +89,9 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
     a0 = block_sum(a0, red);
     sm = block_sum(sm, red);
     cnt = block_sum(cnt, red);
+    cnt0 = block_sum(cnt0, red);
+    // samples at u == 0 (CurveMeta::n_zero) leave the sample arrays when there are few of them
+    const bool divert = cnt0 > 0.0 && cnt0 <= 255.0;
     umin = block_min(umin, red);
     double umax = -block_min(nmax, red);
 
@@ -115,15 +119,16 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
         double mant = frexp(room / a, &e);   // room / a = mant * 2^e, mant in [0.5, 1)
         (void)mant;
         shift = e - 1;                        // 2^shift <= room / a
-        if (shift > 62) shift = 62;
-        if (shift < -62) shift = -62;
+        // every finite fp32 curve fits: a <= n 2^128 and a >= 2^-149
+        if (shift > 200) shift = 200;
+        if (shift < -200) shift = -200;
     }
     const double scale = ldexp(1.0, shift);
 
     // pass 3: ordered compaction + conversion
     if (tid == 0) tile_base = 0;
     __syncthreads();
-    double qsum = 0.0;
+    double qsum = 0.0, qzero = 0.0;
     for (long long b = 0; b < n; b += PREP_THREADS) {
         long long i = b + tid;
         bool ok = false;
@@ -136,6 +141,11 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
             if (ok) {
                 u = __dsub_rn(ti, t0);
                 q = (int)llrint(((double)fi - center) * scale);
+                if (divert && u == 0.0) {
+                    qzero += (double)q;
+                    qsum += (double)q;
+                    ok = false;
+                }
             }
         }
         unsigned bal = __ballot_sync(0xffffffffu, ok);
@@ -161,6 +171,7 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
     const long long tile0 = start / GPFC_TILE + c;   // disjoint per curve: ceil(n/T) <= n/T + 1
     const long long rec0 = (start + c + 1) & ~1LL;   // even, disjoint per curve
     qsum = block_sum(qsum, red);                     // exact: |sum q| < 2^31
+    qzero = block_sum(qzero, red);
     double span_max = 0.0;
     for (int t = warp; t * GPFC_TILE < n_valid; t += PREP_THREADS / 32) {
         const int base = t * GPFC_TILE;
@@ -212,7 +223,9 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
         CurveMeta m;
         m.start = start;
         m.rec0 = rec0;
-        m.pivot = (tile_base > 0) ? __ddiv_rn(__dmul_rn(qsum, ldexp(1.0, -shift)), (double)tile_base) : 0.0;
+        m.pivot = (cnt > 0.0) ? __ddiv_rn(__dmul_rn(qsum, ldexp(1.0, -shift)), cnt) : 0.0;
+        m.n_zero = divert ? (int)cnt0 : 0;
+        m.q_zero = (int)qzero;
         m.tile0 = tile0;
         m.span_max = span_max;
         m.n_valid = tile_base;
@@ -226,16 +239,16 @@ prep_curves_kernel(const double *__restrict__ times, const float *__restrict__ f
 }
 
 // rp[j] = RN(1/P_j) * rows (exact scaling for power-of-two rows), NaN when the
-// period is not finite and positive.  rows = nbins, or 256 when the lane-period kernel
-// folds at 256 (or 1024) rows and merges adjacent rows at write-out (fold_lp.cu).
+// period is not finite and positive.  rows = fold_rows(nbins): the resolution the fold
+// kernel works at (it merges adjacent rows at write-out when nbins is smaller).
 __global__ void prep_periods_kernel(const double *__restrict__ periods, long long nperiods,
-                                    int nbins, double *__restrict__ rp)
+                                    int rows, double *__restrict__ rp)
 {
     long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= nperiods) return;
     double p = periods[j];
     double r = CUDART_NAN;
-    if (period_ok(p)) r = __dmul_rn(__drcp_rn(p), (double)nbins);
+    if (period_ok(p)) r = __dmul_rn(__drcp_rn(p), (double)rows);
     rp[j] = r;
 }
 
@@ -243,16 +256,18 @@ __global__ void prep_periods_kernel(const double *__restrict__ periods, long lon
 
 cudaError_t launch_prep(const double *times, const float *flux, const int64_t *offsets,
                         long long ncurves, const double *t0, double t0_scalar,
-                        const double *periods, long long nperiods, int nbins, Scratch s,
+                        const double *periods, long long nperiods, int rows, Scratch s,
                         cudaStream_t st)
 {
-    if (ncurves > 0)
+    if (ncurves > 0) {
         prep_curves_kernel<<<(unsigned)ncurves, PREP_THREADS, 0, st>>>(times, flux, offsets, t0,
                                                                       t0_scalar, s);
+        note_launch();
+    }
     if (nperiods > 0) {
         unsigned blocks = (unsigned)((nperiods + 255) / 256);
-        prep_periods_kernel<<<blocks, 256, 0, st>>>(periods, nperiods,
-                                                    fold_lp_handles(nbins) ? fold_lp_rows(nbins) : nbins, s.rp);
+        prep_periods_kernel<<<blocks, 256, 0, st>>>(periods, nperiods, rows, s.rp);
+        note_launch();
     }
     return cudaGetLastError();
 }

@@ -320,15 +320,132 @@ def test_flat_and_sparse_profiles_fused_normalise(gp, ref):
 
 
 def test_profile_hooks_count_launches(gp):
+    """gpfc_profile_read: one event pair per fold-kernel launch, and every kernel of the
+    library counted where it is launched (grid, two prepass kernels, fold), for each of the
+    three fold kernels."""
     w = workloads.config0(nperiods=64)
     periods = gp.gpfc_make_period_grid(w.pmin, w.pmax, 64, w.grid_mode)
     t, f, off = dev(w.times), dev(w.flux), dev(w.offsets)
-    gp.gpfc_fold_batch(t, f, off, periods, w.nbins)            # warm-up (one-time probe launch)
+    for nbins in (w.nbins, 1024, 4096, 100):
+        gp.gpfc_profile(True)
+        for _ in range(3):
+            gp.gpfc_make_period_grid(w.pmin, w.pmax, 64, w.grid_mode, out=periods)
+            gp.gpfc_fold_batch(t, f, off, periods, nbins)
+        p = gp.gpfc_profile_read()
+        gp.gpfc_profile(False)
+        assert p["fold_launches"] == 3 and p["kernel_launches"] == 3 * 4, (nbins, p)
+        assert 0.0 < p["fold_kernel_ms"] < 1000.0
     gp.gpfc_profile(True)
-    for _ in range(3):
-        gp.gpfc_make_period_grid(w.pmin, w.pmax, 64, w.grid_mode, out=periods)
-        gp.gpfc_fold_batch(t, f, off, periods, w.nbins)
+    gp.gpfc_fold(t, f, periods, 64)                    # single-curve entry: + the offsets kernel
+    gp.gpfc_normalize(*gp.gpfc_fold(t, f, periods, 64))
     p = gp.gpfc_profile_read()
     gp.gpfc_profile(False)
-    assert p["fold_launches"] == 3 and p["kernel_launches"] == 3 * 4
-    assert 0.0 < p["fold_kernel_ms"] < 1000.0
+    assert p["fold_launches"] == 2 and p["kernel_launches"] == 2 * 4 + 1
+
+
+# ------------------------------------------------------------------ any sample order (gpfc.h)
+
+@pytest.mark.parametrize("nbins", [256, 1024, 4096, 100])
+def test_unsorted_and_duplicate_times(gp, ref, nbins):
+    """gpfc.h: samples may come in any order.  A shuffled Kepler-shaped curve (tiles then span
+    the whole baseline: the kernels take the exact division for every point-period), the same
+    curve with every 7th time stamp duplicated, and a curve sorted in DEScending order: bins,
+    counts and sums identical to the sorted fold, and the slow path is reported."""
+    w = workloads.config1(nperiods=40)
+    rng = np.random.default_rng(11)
+    periods = ref.make_period_grid(w.pmin, w.pmax, w.nperiods)
+    n = 20000
+    t, f = w.times[:n].copy(), w.flux[:n].copy()
+    dup = np.arange(0, n - 1, 7)
+    t[dup] = t[dup + 1]                                  # duplicate time stamps
+    rs, rc, _ = ref.fold(t, f, periods, nbins)
+    perm = rng.permutation(n)
+    gp.gpfc_profile(False)
+    for order in (perm, np.arange(n)[::-1].copy(), np.arange(n)):
+        s, c = gp.gpfc_fold(dev(t[order]), dev(f[order]), dev(periods), nbins)
+        torch.cuda.synchronize()
+        assert np.array_equal(c.cpu().numpy().view(np.uint32), rc)
+        assert np.array_equal(s.cpu().numpy(), rs)       # exact integer sums: order-free
+    counters = gp.gpfc_path_counters()
+    if nbins == 100:
+        assert counters["generic_kernel_calls"] == 3
+    else:
+        assert counters["exact_path_items"] > 0          # the shuffled call took the exact path
+
+
+def test_outputs_with_4_byte_alignment(gp, ref):
+    """Outputs that are contiguous but only 4-byte aligned (a view at offset 1 of a larger
+    buffer) are accepted: scalar stores instead of vector stores."""
+    w = workloads.config2(ncurves=2, nperiods=70)
+    periods = ref.make_period_grid(w.pmin, w.pmax, w.nperiods)
+    for nbins in (64, 256, 1024):
+        r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
+        shape = (w.ncurves, w.nperiods, nbins)
+        nel = int(np.prod(shape))
+        bs = torch.zeros(nel + 3, dtype=torch.float32, device="cuda")
+        bc = torch.zeros(nel + 3, dtype=torch.int32, device="cuda")
+        bn = torch.zeros(nel + 3, dtype=torch.float32, device="cuda")
+        os_, oc, on = (b[1:1 + nel].view(shape) for b in (bs, bc, bn))
+        assert os_.data_ptr() % 16 == 4
+        gp.gpfc_fold_batch(dev(w.times), dev(w.flux), dev(w.offsets), dev(periods), nbins,
+                           out_sum=os_, out_count=oc, out_norm=on)
+        torch.cuda.synchronize()
+        assert np.array_equal(oc.cpu().numpy().view(np.uint32), r["count"])
+        assert np.array_equal(os_.cpu().numpy(), r["sum"])
+        err = np.abs(on.cpu().numpy().astype(np.float64) - r["norm64"])
+        assert np.all(err <= 1e-4 * np.maximum(1.0, np.abs(r["norm64"])))
+        for b in (bs, bc, bn):                            # nothing written outside the view
+            assert float(b[0]) == 0 and float(b[nel + 1]) == 0 and float(b[nel + 2]) == 0
+
+
+def test_fold_batch_in_a_cuda_graph(gp, ref):
+    """Device-pointer calls never synchronise: with a registered workspace the whole step
+    (grid + batched fold + normalise) is captured in a CUDA graph and replayed."""
+    w = workloads.config2(ncurves=2, nperiods=96)
+    t, f, off = dev(w.times), dev(w.flux), dev(w.offsets)
+    shape = (w.ncurves, w.nperiods, w.nbins)
+    periods = torch.empty(w.nperiods, dtype=torch.float64, device="cuda")
+    s = torch.empty(shape, dtype=torch.float32, device="cuda")
+    c = torch.empty(shape, dtype=torch.int32, device="cuda")
+    nrm = torch.empty(shape, dtype=torch.float32, device="cuda")
+    ws = torch.empty(gp.gpfc_workspace_bytes(w.ncurves, w.n_total, w.nperiods, w.nbins),
+                     dtype=torch.uint8, device="cuda")
+    gp.gpfc_set_workspace(ws)
+    try:
+        gp.gpfc_init()
+        g = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(g, stream=side):
+                gp.gpfc_make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode, out=periods)
+                gp.gpfc_fold_batch(t, f, off, periods, w.nbins, out_sum=s, out_count=c, out_norm=nrm)
+        torch.cuda.current_stream().wait_stream(side)
+        for _ in range(2):
+            s.zero_(); c.zero_(); nrm.zero_(); periods.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            pr = ref.make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode)
+            assert np.array_equal(periods.cpu().numpy(), pr)
+            r = ref.fold_batch(w.times, w.flux, w.offsets, pr, w.nbins)
+            assert np.array_equal(c.cpu().numpy().view(np.uint32), r["count"])
+            assert np.array_equal(s.cpu().numpy(), r["sum"])
+    finally:
+        gp.gpfc_set_workspace(None)
+
+
+def test_second_device_if_present(gp, ref):
+    """Per-device library state: the same process folds on cuda:1 after cuda:0."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one CUDA device")
+    w = workloads.config2(ncurves=1, nperiods=64)
+    periods = ref.make_period_grid(w.pmin, w.pmax, w.nperiods)
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, 1024)
+    for d in (0, 1, 0):
+        with torch.cuda.device(d):
+            to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda(d)
+            s, c, _ = gp.gpfc_fold_batch(to(w.times), to(w.flux), to(w.offsets), to(periods), 1024,
+                                         want=("sum", "count"))
+            torch.cuda.synchronize(d)
+            assert np.array_equal(c.cpu().numpy().view(np.uint32), r["count"])
+            assert np.array_equal(s.cpu().numpy(), r["sum"])
