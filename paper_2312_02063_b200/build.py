@@ -39,7 +39,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not os.path.exists(nvcc):
         nvcc = "nvcc"
     tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [nvcc, *NVCC_FLAGS, "-o", tmp, *sources()]
+    extra = os.environ.get("GPFC_NVCC_EXTRA", "").split()      # experiments: -D switches of the kernels
+    cmd = [nvcc, *NVCC_FLAGS, *extra, "-o", tmp, *sources()]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.check_call(cmd)

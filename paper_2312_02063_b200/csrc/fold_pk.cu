@@ -42,6 +42,10 @@ constexpr int PK_SCR_BYTES = 28672;
 constexpr int PK_CTR_OFF = PK_SCR_OFF + PK_SCR_BYTES;
 constexpr int PK_SMEM_BYTES = PK_CTR_OFF + 16;
 constexpr int PK_FLUSH_TILES = 511;               // 65,408 samples between count flushes
+#ifndef PK_UNROLL
+#define PK_UNROLL 4
+#endif
+constexpr int PK_UNROLL_C = PK_UNROLL;          // iterations (4 samples per lane each) unrolled in the fold loop
 constexpr int PK_NSEG = 16;                       // row segments of the merge scan
 // scratch, fold phase: int2 stage[PK_WARPS][PK_GRAN]                       12,288 B
 // scratch, bins epilogue: double ps1, ps2 [PK_WARPS][32]; int pkk [PK_WARPS][32];
@@ -202,10 +206,12 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
         if (!fast && tid == 0 && a.stats) atomicAdd(a.stats + 0, 1ull);
         const double per_exact = (valid && !fast) ? a.periods[j] : 1.0;
 
+        // segments between count flushes: equal shares of at most PK_FLUSH_TILES tiles
         const int nseg = (ntiles + PK_FLUSH_TILES - 1) / PK_FLUSH_TILES;
+        const int tps = (nseg > 1) ? (ntiles + nseg - 1) / nseg : ntiles;
         for (int seg = 0; seg < nseg; ++seg) {
-            const int t_lo = seg * PK_FLUSH_TILES;
-            const int t_n = min(ntiles - t_lo, PK_FLUSH_TILES);
+            const int t_lo = seg * tps;
+            const int t_n = min(ntiles - t_lo, tps);
             if (fast) {
                 // work units: whole anchor tiles first, the last 2 * PK_WARPS tiles in halves
                 const int nfull = max(0, t_n - 2 * PK_WARPS);
@@ -243,7 +249,7 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                         if (g0 + PK_GRAN + 2 * lane < cnt) nx = __ldg(src4 + (g0 + PK_GRAN) / 2 + lane);
                         if (gc == PK_GRAN) {
                             // slot s takes the sample pairs s, s + SL, s + 2 SL, ...
-#pragma unroll 1
+#pragma unroll(PK_UNROLL_C)
                             for (int g = 0; g < PK_GRAN / 2; g += 2 * SL) {
                                 const int4 ra = stage4[g + slot], rb = stage4[g + SL + slot];
                                 pk_update<ROWLOG, IMM>((double)(unsigned)ra.x, ra.y, rps, C, p4, one, sbase, gmin);
@@ -330,7 +336,28 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                 __syncthreads();
             }
         }
-        const unsigned *sd = (nseg > 1) ? side : nullptr;
+        // Counts that were flushed go back into the packed half-words if every row pair of
+        // every period holds fewer than 65,536 points (always, unless nearly the whole curve
+        // sits in one pair of rows): the epilogues then read shared memory only.
+        const unsigned *sd = nullptr;
+        if (nseg > 1) {
+            int over = 0;
+            for (int i = tid; i < HALF * PL; i += PK_THREADS) {
+                const unsigned w = H[PK_CNT_OFF / 4 + i];
+                const unsigned slo = __ldcg(side + i), shi = __ldcg(side + i + HALF * PL);
+                over |= ((w & 0xffffu) + slo + shi > 0xffffu) ? 1 : 0;
+            }
+            over = __syncthreads_or(over);
+            if (over) {
+                sd = side;
+            } else {
+                for (int i = tid; i < HALF * PL; i += PK_THREADS) {
+                    const unsigned slo = __ldcg(side + i), shi = __ldcg(side + i + HALF * PL);
+                    H[PK_CNT_OFF / 4 + i] += slo + shi + (shi << 16);
+                }
+                __syncthreads();
+            }
+        }
         const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
         const bool ok = live && valid;
 
