@@ -234,7 +234,7 @@ int gpfc_profile(int enable);
 int gpfc_profile_read(double *fold_kernel_ms, int64_t *fold_launches, int64_t *kernel_launches);
 
 /*
- * Which slow paths ran since the last gpfc_profile() call (out: host int64[4]):
+ * Which slow paths ran since the last gpfc_profile() call (out: host int64[8]):
  *   [0] fold calls of this thread that used the generic kernel (nbins not a power of two
  *       in 32 ... 4096: one CTA per (curve, period), true division for every point-period)
  *   [1] work items (curve x group of periods) of this DEVICE that took the exact division for
@@ -242,6 +242,10 @@ int gpfc_profile_read(double *fold_kernel_ms, int64_t *fold_launches, int64_t *k
  *       sampling interval
  *   [2] guard-band re-checks (lane x tile) of this device: normal, ~1e-4 of the tiles
  *   [3] gpfc_fold_two_tier calls of this thread that could not fuse fold and merge
+ *   [4] work items of this device (nbins >= 512, curves of more than 65,408 samples) folded
+ *       twice because more than 65,535 points of a period fell into one pair of rows: the
+ *       second pass flushes the packed 16-bit counts to a 32-bit side array
+ *   [5..7] reserved (0)
  * Synchronises the calling thread's stream.
  */
 int gpfc_path_counters(int64_t *out);

@@ -244,11 +244,12 @@ def gpfc_init() -> None:
 
 
 def gpfc_path_counters() -> dict:
-    out = (ctypes.c_int64 * 4)()
+    out = (ctypes.c_int64 * 8)()
     _use_current_stream()
     _check(lib().gpfc_path_counters(out), "gpfc_path_counters")
     return {"generic_kernel_calls": out[0], "exact_path_items": out[1],
-            "guard_band_rechecks": out[2], "unfused_two_tier_calls": out[3]}
+            "guard_band_rechecks": out[2], "unfused_two_tier_calls": out[3],
+            "count_overflow_refolds": out[4]}
 
 
 def gpfc_make_period_grid_host(pmin, pmax, nperiods, mode_flags=0):

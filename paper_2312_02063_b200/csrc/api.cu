@@ -571,7 +571,7 @@ int gpfc_path_counters(int64_t *out)
 {
     if (!out) return fail(GPFC_ERR_INVALID_ARG, "out is NULL%s");
     out[0] = g_ts.generic_launches;
-    out[1] = out[2] = 0;
+    out[1] = out[2] = out[4] = out[5] = out[6] = out[7] = 0;
     out[3] = g_ts.unfused_two_tier;
     const gpfc::DeviceInfo *di = nullptr;
     cudaError_t e = gpfc::device_info(&di);
@@ -581,6 +581,7 @@ int gpfc_path_counters(int64_t *out)
     if (e != cudaSuccess) return cuda_fail(e, "gpfc_path_counters");
     out[1] = (int64_t)h[0];
     out[2] = (int64_t)h[1];
+    out[4] = (int64_t)h[2];
     return GPFC_OK;
 }
 

@@ -82,7 +82,8 @@ struct FoldArgs {
 struct DeviceInfo {
     int num_sms;
     unsigned long long *stats;    // device counters: [0] work items folded with the exact formula
-                                  // for every point-period, [1] guard-band re-checks (lane x tile)
+                                  // for every point-period, [1] guard-band re-checks (lane x tile),
+                                  // [2] work items folded twice (packed 16-bit count overflow)
 };
 cudaError_t device_info(const DeviceInfo **out);
 void note_launch(int n = 1);      // per-thread kernel-launch counter (gpfc_profile_read)

@@ -38,7 +38,7 @@ constexpr int PK_HIST_BYTES = 196608;
 constexpr int PK_HIST_WORDS = PK_HIST_BYTES / 4;
 constexpr int PK_CELLS = 32768;                   // ROWS * PL, every variant
 constexpr int PK_SCR_OFF = PK_HIST_BYTES;         // scratch: staging | statistics partials | merge
-constexpr int PK_SCR_BYTES = 28672;
+constexpr int PK_SCR_BYTES = 35072;
 constexpr int PK_CTR_OFF = PK_SCR_OFF + PK_SCR_BYTES;
 constexpr int PK_SMEM_BYTES = PK_CTR_OFF + 16;
 constexpr int PK_FLUSH_TILES = 511;               // 65,408 samples between count flushes
@@ -46,7 +46,6 @@ constexpr int PK_FLUSH_TILES = 511;               // 65,408 samples between coun
 #define PK_UNROLL 4
 #endif
 constexpr int PK_UNROLL_C = PK_UNROLL;          // iterations (4 samples per lane each) unrolled in the fold loop
-constexpr int PK_NSEG = 16;                       // row segments of the merge scan
 // scratch, fold phase: int2 stage[PK_WARPS][PK_GRAN]                       12,288 B
 // scratch, bins epilogue: double ps1, ps2 [PK_WARPS][32]; int pkk [PK_WARPS][32];
 //                         double mu[32], isd[32]; int kk[32]                16,000 B
@@ -56,13 +55,11 @@ constexpr int PK_PKK_OFF = PK_PS2_OFF + PK_WARPS * 32 * 8;
 constexpr int PK_MU_OFF = PK_PKK_OFF + PK_WARPS * 32 * 4;
 constexpr int PK_ISD_OFF = PK_MU_OFF + 32 * 8;
 constexpr int PK_KK_OFF = PK_ISD_OFF + 32 * 8;
-// scratch, merge epilogue: unsigned segc[PK_NSEG][PL]; int segq[PK_NSEG][PL] (4 KB at most),
-//                          unsigned ntot[PL]; double scum[PL][nb2 + 1]      <= 24,448 B
-constexpr int PK_SEGC_OFF = PK_SCR_OFF;
-constexpr int PK_SEGQ_OFF = PK_SEGC_OFF + PK_NSEG * 32 * 4;
-constexpr int PK_NTOT_OFF = PK_SEGQ_OFF + PK_NSEG * 32 * 4;      // unsigned ntot[32]
-constexpr int PK_SCUM_OFF = PK_NTOT_OFF + 32 * 4;
-constexpr int PK_SCUM_BYTES = PK_SCR_OFF + PK_SCR_BYTES - PK_SCUM_OFF;
+// scratch, merge epilogue: cumulative count / integer flux in front of every mini-chunk
+// (32 or 16 KB), warp totals [PK_WARPS][PL] (6 KB at most); the cumulative flux at the
+// boundaries goes over the histogram: [nb2 + 1][PL] doubles, PL * nb2 <= PK_MG_MAX
+constexpr int PK_MG_MAX = 2048;
+static_assert((PK_MG_MAX + 32) * 8 <= PK_HIST_BYTES, "cumulative flux table fits over the histogram");
 static_assert(PK_KK_OFF + 32 * 4 <= PK_SCR_OFF + PK_SCR_BYTES, "bins-epilogue scratch");
 static_assert(PK_WARPS * PK_GRAN * 8 <= PK_SCR_BYTES, "staging scratch");
 static_assert(PK_SMEM_BYTES <= 227 * 1024, "shared memory budget");
@@ -206,8 +203,15 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
         if (!fast && tid == 0 && a.stats) atomicAdd(a.stats + 0, 1ull);
         const double per_exact = (valid && !fast) ? a.periods[j] : 1.0;
 
-        // segments between count flushes: equal shares of at most PK_FLUSH_TILES tiles
-        const int nseg = (ntiles + PK_FLUSH_TILES - 1) / PK_FLUSH_TILES;
+        // Count flushes.  A curve of more than PK_FLUSH_TILES tiles could overflow a packed
+        // half-word, but only if more than 65,535 of its points share one pair of rows: the
+        // first attempt folds it without flushes and checks afterwards (the low half-words of
+        // a period add up to n_valid exactly iff none of them wrapped); if one did, the
+        // histogram is cleared and the item is folded again in segments of at most
+        // PK_FLUSH_TILES tiles with the counts flushed to the 32-bit side array in between.
+        const unsigned *sd = nullptr;
+        for (int attempt = 0;; ++attempt) {
+        const int nseg = (fast && attempt == 0) ? 1 : (ntiles + PK_FLUSH_TILES - 1) / PK_FLUSH_TILES;
         const int tps = (nseg > 1) ? (ntiles + nseg - 1) / nseg : ntiles;
         for (int seg = 0; seg < nseg; ++seg) {
             const int t_lo = seg * tps;
@@ -339,7 +343,7 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
         // Counts that were flushed go back into the packed half-words if every row pair of
         // every period holds fewer than 65,536 points (always, unless nearly the whole curve
         // sits in one pair of rows): the epilogues then read shared memory only.
-        const unsigned *sd = nullptr;
+        sd = nullptr;
         if (nseg > 1) {
             int over = 0;
             for (int i = tid; i < HALF * PL; i += PK_THREADS) {
@@ -357,6 +361,26 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                 }
                 __syncthreads();
             }
+            break;
+        }
+        if (ntiles <= PK_FLUSH_TILES || !fast) break;
+        {
+            // optimistic attempt of a long curve: did a half-word wrap?  Thread tid only meets
+            // count words of its own period p (PK_THREADS is a multiple of PL).
+            unsigned *chk = reinterpret_cast<unsigned *>(smem + PK_SCR_OFF);     // [PK_WARPS][32]
+            unsigned lo_sum = 0;
+            for (int i = tid; i < HALF * PL; i += PK_THREADS) lo_sum += H[PK_CNT_OFF / 4 + i] & 0xffffu;
+            chk[tid] = lo_sum;
+            __syncthreads();
+            unsigned tot = 0;
+            for (int i = p; i < PK_THREADS; i += PL) tot += chk[i];
+            const int wrapped = __syncthreads_or((live && valid && tot != (unsigned)n) ? 1 : 0);
+            if (!wrapped) break;
+            if (a.stats && tid == 0) atomicAdd(a.stats + 2, 1ull);
+            for (int i = tid; i < PK_HIST_WORDS; i += PK_THREADS) H[i] = 0u;
+            if (tid == 0) *ctr = 0;
+            __syncthreads();
+        }
         }
         const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
         const bool ok = live && valid;
@@ -503,15 +527,25 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
             //   boundary b lies in the first row k with C(k) >= target_b (C = cumulative count),
             //   Scum_b = S(k-1) + ((target_b - C(k-1)) / count_k) sum_k,
             //   mean_b = (Scum_b - Scum_{b-1}) / per.
-            // The rows are scanned in PK_NSEG segments (one warp each, 64 steps of SL rows: the
-            // SL slots read SL consecutive rows, conflict-free); cumulative counts and integer
-            // sums are exact (|any partial sum of q| < 2^31 by the choice of the scale).
-            unsigned *segc = reinterpret_cast<unsigned *>(smem + PK_SEGC_OFF);
-            int *segq = reinterpret_cast<int *>(smem + PK_SEGQ_OFF);
-            unsigned *ntot_s = reinterpret_cast<unsigned *>(smem + PK_NTOT_OFF);
-            double *scum = reinterpret_cast<double *>(smem + PK_SCUM_OFF);
+            // Phases: every thread (chunk c, period p) adds up its 2-6 mini-chunks of MCR rows ->
+            // prefix over threads: cumulative count / integer flux in front of every mini-chunk
+            // (exact: |any partial sum of q| < 2^31 by the choice of the scale) -> one
+            // (boundary, period) per lane: binary search of the mini-chunk, walk of at most
+            // MCR rows, the fp64 part -> means, statistics, write-out.
+            constexpr int MCR = (PL == 8) ? 8 : 16;        // rows per mini-chunk
+            constexpr int NMC = ROWS / MCR;                // mini-chunks: 512 / 128 / 64
+            constexpr int NCH = PK_THREADS / PL;           // threads per period: 96 / 48 / 24
+            constexpr int MNUM = NMC / (NCH / 3);          // a thread owns MNUM / 3 mini-chunks
+            constexpr int MPT = MNUM / 3 + 1;              // ... at most (6 / 3 / 3)
+            static_assert(NCH % 3 == 0 && (NCH / 3) * MNUM == NMC, "mini-chunks split evenly");
+            static_assert(NMC * PL * 8 + PK_WARPS * PL * 8 <= PK_SCR_BYTES, "merge-epilogue scratch");
+            unsigned *ec = reinterpret_cast<unsigned *>(smem + PK_SCR_OFF);             // [NMC][PL]
+            int *eq = reinterpret_cast<int *>(smem + PK_SCR_OFF) + NMC * PL;            // [NMC][PL]
+            unsigned *wtc = reinterpret_cast<unsigned *>(smem + PK_SCR_OFF) + 2 * NMC * PL;   // [warp][PL]
+            int *wtq = reinterpret_cast<int *>(wtc) + PK_WARPS * PL;                    // [warp][PL]
+            double *part = reinterpret_cast<double *>(wtc);                             // [warp][PL], later
+            double *scum = reinterpret_cast<double *>(smem);                            // [nb2 + 1][PL], over H
             const int nb2 = a.nb2;
-            constexpr int RPS = ROWS / PK_NSEG;            // rows per segment
             if (cm.n_zero > 0) {
                 // the samples at u == 0 (CurveMeta::n_zero, at most 255) belong to row 0
                 if (tid < PL) {
@@ -520,145 +554,155 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                 }
                 __syncthreads();
             }
-            constexpr int STEPS = RPS / SL;                // 64
-            if (warp < PK_NSEG) {
-                unsigned tc = 0;
-                int tq = 0;
-                const int r0 = warp * RPS + slot;
-#pragma unroll 4
-                for (int i = 0; i < STEPS; ++i) {
-                    const int row = r0 + i * SL;
-                    tc += pk_count<ROWLOG>(H, sd, row, p);
-                    tq += (int)H[row * PL + p];
-                }
+            const int ch = warp * SL + slot;
+            const int m_lo = (ch * MNUM) / 3, m_hi = ((ch + 1) * MNUM) / 3;
+            // phase 1: totals of this thread's mini-chunks (slot s starts s rows into each, so
+            // the SL slots of a warp read rows that differ mod SL: conflict-free)
+            unsigned lc[MPT];
+            int lq[MPT];
+            unsigned tc = 0;
+            int tq = 0;
 #pragma unroll
-                for (int o = PL; o < 32; o <<= 1) {
-                    tc += __shfl_xor_sync(0xffffffffu, tc, o);
-                    tq += __shfl_xor_sync(0xffffffffu, tq, o);
+            for (int k = 0; k < MPT; ++k) {
+                unsigned c1 = 0;
+                int q1 = 0;
+                if (m_lo + k < m_hi) {
+#pragma unroll
+                    for (int i = 0; i < MCR; ++i) {
+                        const int row = (m_lo + k) * MCR + ((i + slot) & (MCR - 1));
+                        c1 += pk_count<ROWLOG>(H, sd, row, p);
+                        q1 += (int)H[row * PL + p];
+                    }
                 }
-                if (slot == 0) {
-                    segc[warp * PL + p] = tc;
-                    segq[warp * PL + p] = tq;
+                lc[k] = tc;            // exclusive prefix inside the thread
+                lq[k] = tq;
+                tc += c1;
+                tq += q1;
+            }
+            unsigned ci = tc;
+            int qi = tq;
+#pragma unroll
+            for (int o = 1; o < SL; o <<= 1) {
+                const unsigned cu = __shfl_up_sync(0xffffffffu, ci, o * PL);
+                const int qu = __shfl_up_sync(0xffffffffu, qi, o * PL);
+                if (slot >= o) {
+                    ci += cu;
+                    qi += qu;
                 }
             }
+            if (slot == SL - 1) {
+                wtc[warp * PL + p] = ci;
+                wtq[warp * PL + p] = qi;
+            }
             __syncthreads();
-            if (warp < PK_NSEG) {
-                unsigned cb = 0, ntot = 0;       // points before this segment, total
-                int qb = 0;                      // integer flux before this segment
-                for (int s = 0; s < PK_NSEG; ++s) {
-                    const unsigned c = segc[s * PL + p];
-                    if (s < warp) {
-                        cb += c;
-                        qb += segq[s * PL + p];
-                    }
-                    ntot += c;
+            // phase 2: points / integer flux in front of this thread, total of the period;
+            // table of the cumulative values in front of every mini-chunk
+            unsigned cb = ci - tc, ntot = 0;
+            int qb = qi - tq;
+            for (int w = 0; w < PK_WARPS; ++w) {
+                const unsigned c = wtc[w * PL + p];
+                if (w < warp) {
+                    cb += c;
+                    qb += wtq[w * PL + p];
                 }
-                if (!ok) ntot = 0;
-                const double total = (double)ntot;
-                const double per = __ddiv_rn(total, (double)nb2);
-                double *sc = scum + p * (nb2 + 1);
-                const bool act = ntot > 0u;      // per lane (period); the shuffles below are warp-wide
-                // next boundary not yet emitted, its target and thr = ceil(target):
-                // C >= target  <=>  C >= thr for an integer C
-                int b = nb2;
-                double target = 0.0;
-                unsigned thr = 0xffffffffu;
-                auto set_b = [&](int bb) {
-                    b = bb;
+                ntot += c;
+            }
+            if (!ok) ntot = 0;
+#pragma unroll
+            for (int k = 0; k < MPT; ++k)
+                if (m_lo + k < m_hi) {
+                    ec[(m_lo + k) * PL + p] = cb + lc[k];
+                    eq[(m_lo + k) * PL + p] = qb + lq[k];
+                }
+            __syncthreads();
+            // phase 3: boundary b of period p: first row k with C(k) >= thr_b = ceil(target_b)
+            // (C >= target <=> C >= thr for an integer C), then the cumulative flux there
+            const double total = (double)ntot;
+            const double per = __ddiv_rn(total, (double)nb2);
+            double sv[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                sv[k] = 0.0;
+                const int b = ch + k * NCH;
+                if (b < nb2 && ntot > 0u) {
+                    const double target = (b == nb2 - 1) ? total : __dmul_rn(per, (double)(b + 1));
+                    const unsigned thr = (unsigned)ceil(target);
+                    int m = 0;                           // last mini-chunk with fewer than thr points in front
+#pragma unroll
+                    for (int step = NMC / 2; step >= 1; step >>= 1)
+                        if (ec[(m + step) * PL + p] < thr) m += step;
+                    unsigned cbef = ec[m * PL + p], cnt = 0;
+                    int qbef = eq[m * PL + p], q = 0;
+                    int row = m * MCR;
+                    for (int i = 0; i < MCR; ++i, ++row) {
+                        cnt = pk_count<ROWLOG>(H, sd, row, p);
+                        q = (int)H[row * PL + p];
+                        if (cbef + cnt >= thr || i == MCR - 1) break;
+                        cbef += cnt;
+                        qbef += q;
+                    }
+                    const double ck = (double)cnt, cbd = (double)cbef;
+                    const double sbef = __dadd_rn(__dmul_rn((double)qbef, inv_scale), __dmul_rn(cbd, center));
+                    const double sk = __dadd_rn(__dmul_rn((double)q, inv_scale), __dmul_rn(ck, center));
+                    double frac = (cnt > 0u) ? __ddiv_rn(__dsub_rn(target, cbd), ck) : 0.0;
+                    frac = fmin(fmax(frac, 0.0), 1.0);
+                    sv[k] = __dadd_rn(sbef, __dmul_rn(frac, sk));
+                }
+            }
+            __syncthreads();   // the histogram has been read for the last time: scum goes over it
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const int b = ch + k * NCH;
+                if (b < nb2) scum[(b + 1) * PL + p] = sv[k];
+            }
+            if (ch == 0) scum[p] = 0.0;
+            __syncthreads();
+            // phase 4: means; mean and population std over the nb2 bins, summed
+            // in a fixed order (slots by shuffle, warps in order)
+            double mv[3], s1 = 0.0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                mv[k] = 0.0;
+                const int b = ch + k * NCH;
+                if (b < nb2 && ntot > 0u)
+                    mv[k] = __ddiv_rn(__dsub_rn(scum[(b + 1) * PL + p], scum[b * PL + p]), per);
+                s1 += mv[k];
+            }
+#pragma unroll
+            for (int o = PL; o < 32; o <<= 1) s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+            if (slot == 0) part[warp * PL + p] = s1;
+            __syncthreads();
+            double mu = 0.0;
+            for (int w = 0; w < PK_WARPS; ++w) mu += part[w * PL + p];
+            mu = __ddiv_rn(mu, (double)nb2);
+            double s2 = 0.0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double d = (ch + k * NCH < nb2) ? __dsub_rn(mv[k], mu) : 0.0;
+                s2 += __dmul_rn(d, d);
+            }
+#pragma unroll
+            for (int o = PL; o < 32; o <<= 1) s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+            __syncthreads();
+            if (slot == 0) part[warp * PL + p] = s2;
+            __syncthreads();
+            if (live) {
+                double vacc = 0.0;
+                for (int w = 0; w < PK_WARPS; ++w) vacc += part[w * PL + p];
+                const double sdv = sqrt(__ddiv_rn(vacc, (double)nb2));
+                const bool flat = (nb2 < 2) || !(sdv > 0.0);
+                const long long off = (curve * a.nperiods + j) * nb2;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const int b = ch + k * NCH;
                     if (b < nb2) {
-                        target = (b == nb2 - 1) ? total : __dmul_rn(per, (double)(b + 1));
-                        thr = (unsigned)ceil(target);
-                    } else {
-                        thr = 0xffffffffu;
-                    }
-                };
-                for (int i = 0; i < STEPS; ++i) {
-                    const int row = warp * RPS + i * SL + slot;
-                    const unsigned c = pk_count<ROWLOG>(H, sd, row, p);
-                    const int q = (int)H[row * PL + p];
-                    // inclusive prefix over the SL slots of this step (slot s = lanes s * PL + p)
-                    unsigned ci = c;
-                    int qi = q;
-#pragma unroll
-                    for (int o = 1; o < SL; o <<= 1) {
-                        const unsigned cu = __shfl_up_sync(0xffffffffu, ci, o * PL);
-                        const int qu = __shfl_up_sync(0xffffffffu, qi, o * PL);
-                        if (slot >= o) {
-                            ci += cu;
-                            qi += qu;
+                        float om = 0.f, on = 0.f;
+                        if (ntot > 0u) {
+                            om = (float)mv[k];
+                            on = (float)(flat ? mu : __dadd_rn(mu, __ddiv_rn(__dsub_rn(mv[k], mu), sdv)));
                         }
-                    }
-                    const unsigned cbef = cb + ci - c, cinc = cb + ci;     // C(row - 1), C(row)
-                    const int qbef = qb + qi - q;
-                    cb += __shfl_sync(0xffffffffu, ci, (SL - 1) * PL + p);
-                    qb += __shfl_sync(0xffffffffu, qi, (SL - 1) * PL + p);
-                    if (!act) continue;
-                    if (i == 0) {
-                        // first boundary whose target lies beyond the points before this row
-                        int bb = (int)floor(__ddiv_rn((double)cbef, per)) - 1;
-                        if (bb < 0 || cbef == 0u) bb = 0;
-                        set_b(bb);
-                    }
-                    // boundaries reached by earlier rows (other slots, other segments)
-                    while (thr <= cbef) set_b(b + 1);
-                    const bool last = (row == ROWS - 1);
-                    if (b < nb2 && (last || thr <= cinc)) {
-                        const double ck = (double)c, cbd = (double)cbef;
-                        const double sbef = __dadd_rn(__dmul_rn((double)qbef, inv_scale),
-                                                      __dmul_rn(cbd, center));
-                        const double sk = __dadd_rn(__dmul_rn((double)q, inv_scale),
-                                                    __dmul_rn(ck, center));
-                        do {
-                            double frac = (c > 0u) ? __ddiv_rn(__dsub_rn(target, cbd), ck) : 0.0;
-                            frac = fmin(fmax(frac, 0.0), 1.0);
-                            sc[b + 1] = __dadd_rn(sbef, __dmul_rn(frac, sk));
-                            set_b(b + 1);
-                        } while (b < nb2 && (last || thr <= cinc));
-                    }
-                }
-                if (warp == 0 && slot == 0) {
-                    sc[0] = 0.0;
-                    ntot_s[p] = ntot;
-                }
-            }
-            __syncthreads();
-            // means, optional normalisation (mean kept, population std 1 over the nb2 bins):
-            // one warp per period, same arithmetic as merge.cu
-            for (int pp = warp; pp < PL; pp += PK_WARPS) {
-                const long long jj = p0 + pp;
-                if (jj >= a.nperiods) continue;
-                const unsigned ntot = ntot_s[pp];
-                const long long off = (curve * a.nperiods + jj) * nb2;
-                if (ntot == 0u) {
-                    for (int bb = lane; bb < nb2; bb += 32) {
-                        if (a.out_mean2) a.out_mean2[off + bb] = 0.f;
-                        if (a.out_norm2) a.out_norm2[off + bb] = 0.f;
-                    }
-                    continue;
-                }
-                const double per = __ddiv_rn((double)ntot, (double)nb2);
-                const double *sc = scum + pp * (nb2 + 1);
-                double acc = 0.0;
-                for (int bb = lane; bb < nb2; bb += 32) {
-                    const double m = __ddiv_rn(__dsub_rn(sc[bb + 1], sc[bb]), per);
-                    if (a.out_mean2) a.out_mean2[off + bb] = (float)m;
-                    acc += m;
-                }
-                if (a.out_norm2) {
-                    acc = warp_sum(acc);
-                    const double mu = __ddiv_rn(acc, (double)nb2);
-                    double vacc = 0.0;
-                    for (int bb = lane; bb < nb2; bb += 32) {
-                        const double d = __dsub_rn(__ddiv_rn(__dsub_rn(sc[bb + 1], sc[bb]), per), mu);
-                        vacc += __dmul_rn(d, d);
-                    }
-                    vacc = warp_sum(vacc);
-                    const double sdv = sqrt(__ddiv_rn(vacc, (double)nb2));
-                    const bool flat = (nb2 < 2) || !(sdv > 0.0);
-                    for (int bb = lane; bb < nb2; bb += 32) {
-                        const double m = __ddiv_rn(__dsub_rn(sc[bb + 1], sc[bb]), per);
-                        const double o = flat ? mu : __dadd_rn(mu, __ddiv_rn(__dsub_rn(m, mu), sdv));
-                        a.out_norm2[off + bb] = (float)o;
+                        if (a.out_mean2) a.out_mean2[off + b] = om;
+                        if (a.out_norm2) a.out_norm2[off + b] = on;
                     }
                 }
             }
@@ -712,8 +756,7 @@ int fold_pk_rows(int nbins) { return nbins <= 1024 ? 1024 : nbins; }
 bool fold_pk_can_merge(int nbins, int nb2)
 {
     if (!(nbins == 1024 || nbins == 2048 || nbins == 4096) || nb2 < 1) return false;
-    const int pl = 32768 / nbins;
-    return (size_t)pl * (size_t)(nb2 + 1) * 8 <= (size_t)PK_SCUM_BYTES;
+    return (32768 / nbins) * nb2 <= PK_MG_MAX;
 }
 
 size_t fold_pk_side_bytes(int sms) { return (size_t)sms * PK_CELLS * sizeof(unsigned); }

@@ -134,7 +134,8 @@ def check_fused(gp, ref, times, flux, periods, nb1, nb2, t0=None, offsets=None, 
     return mean, norm
 
 
-@pytest.mark.parametrize("nb1,nb2", [(4096, 256), (2048, 128), (1024, 64), (4096, 300), (4096, 1)])
+@pytest.mark.parametrize("nb1,nb2", [(4096, 256), (2048, 128), (1024, 64), (4096, 200), (4096, 1),
+                                     (2048, 100), (1024, 33)])
 def test_fused_two_tier_matches_oracle(gp, ref, nb1, nb2):
     """gpfc_fold_two_tier (one kernel: fold at nb1 rows, equal-count merge from the exact sums
     in shared memory) against fold + gpfc_ref_two_tier_merge + normalise of the oracle:
@@ -189,4 +190,5 @@ def test_two_tier_unfused_fallback(gp, ref):
     check_fused(gp, ref, w.times, w.flux, periods, 512, 64)
     check_fused(gp, ref, w.times, w.flux, periods, 1000, 100)
     check_fused(gp, ref, w.times, w.flux, periods, 4096, 1024)
-    assert gp.gpfc_path_counters()["unfused_two_tier_calls"] == 3
+    check_fused(gp, ref, w.times, w.flux, periods, 4096, 300)
+    assert gp.gpfc_path_counters()["unfused_two_tier_calls"] == 4
