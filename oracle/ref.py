@@ -16,6 +16,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "gpfc_ref.c")
+_SRCS = [_SRC, os.path.join(_HERE, "gpfc_ref_sim.c")]
 _LIB = os.path.join(_HERE, "libgpfc_ref.so")
 
 GRID_UNIFORM_FREQUENCY = 0
@@ -29,10 +30,10 @@ CFLAGS = ["-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-shared", "
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (no FMA contraction).  Returns the .so path."""
     if (not force and os.path.exists(_LIB)
-            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+            and all(os.path.getmtime(_LIB) >= os.path.getmtime(f) for f in _SRCS)):
         return _LIB
     tmp = _LIB + ".tmp.%d" % os.getpid()
-    subprocess.check_call(["gcc", *CFLAGS, "-o", tmp, _SRC, "-lm"])
+    subprocess.check_call(["gcc", *CFLAGS, "-o", tmp, *_SRCS, "-lm"])
     os.replace(tmp, _LIB)
     return _LIB
 
@@ -63,6 +64,20 @@ def lib() -> ctypes.CDLL:
                                           c_dp, c_dp, c_dp, c_dp, c_dp]
         L.gpfc_ref_two_tier_merge.argtypes = [c_dp, c_dp, ctypes.c_int, ctypes.c_int,
                                               c_dp, c_dp]
+        L.gpfc_ref_philox4x32_10.argtypes = [c_dp, c_dp, c_dp]
+        L.gpfc_ref_philox4x32_10.restype = None
+        for name in ("gpfc_ref_ln", "gpfc_ref_cos2pi"):
+            getattr(L, name).restype = ctypes.c_double
+            getattr(L, name).argtypes = [ctypes.c_double]
+        L.gpfc_ref_u32_to_unit.restype = ctypes.c_double
+        L.gpfc_ref_u32_to_unit.argtypes = [ctypes.c_uint32]
+        L.gpfc_ref_u52_to_unit.restype = ctypes.c_double
+        L.gpfc_ref_u52_to_unit.argtypes = [ctypes.c_uint32, ctypes.c_uint32]
+        L.gpfc_ref_normal.restype = ctypes.c_double
+        L.gpfc_ref_normal.argtypes = [ctypes.c_uint64, ctypes.c_uint32, ctypes.c_uint32]
+        L.gpfc_ref_lc_params_default.argtypes = [c_dp]
+        L.gpfc_ref_make_light_curves.argtypes = [ctypes.c_uint64, ctypes.c_int64, ctypes.c_int64,
+                                                 c_dp, c_dp, c_dp, c_dp]
         _lib = L
     return _lib
 
@@ -208,3 +223,64 @@ def two_tier_merge(fine_sum64, fine_count, nb2):
                                            _p(osum[i]), _p(omean[i])),
              "gpfc_ref_two_tier_merge")
     return osum.reshape(lead + (nb2,)), omean.reshape(lead + (nb2,))
+
+
+# ---- synthetic light-curve generator (oracle/gpfc_ref_sim.c)
+LC_CENTERED = 1
+LC_NO_NOISE = 2
+LC_PARAM_NAMES = ("period", "duration", "sigma", "depth", "ratio_r", "epoch", "snr", "has_transit")
+
+
+class LcParams(ctypes.Structure):
+    """Mirror of gpfc_ref_lc_params (field order and types as in gpfc_ref_sim.c)."""
+    _fields_ = [(k, ctypes.c_double) for k in (
+        "period_lo", "period_hi", "duration_lo", "duration_hi", "ratio_lo", "ratio_hi",
+        "sigma_lo", "sigma_hi", "snr_lo", "snr_hi", "transit_fraction", "cadence", "t_start")]
+    _fields_ += [("flags", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+def lc_params_default(**over) -> LcParams:
+    prm = LcParams()
+    _chk(lib().gpfc_ref_lc_params_default(ctypes.byref(prm)), "gpfc_ref_lc_params_default")
+    for k, v in over.items():
+        setattr(prm, k, v)
+    return prm
+
+
+def philox4x32_10(ctr, key) -> np.ndarray:
+    ctr = _arr(ctr, np.uint32)
+    key = _arr(key, np.uint32)
+    out = np.empty(4, np.uint32)
+    lib().gpfc_ref_philox4x32_10(_p(ctr), _p(key), _p(out))
+    return out
+
+
+def ln(u: float) -> float:
+    return float(lib().gpfc_ref_ln(float(u)))
+
+
+def cos2pi(v: float) -> float:
+    return float(lib().gpfc_ref_cos2pi(float(v)))
+
+
+def u32_to_unit(x: int) -> float:
+    return float(lib().gpfc_ref_u32_to_unit(int(x)))
+
+
+def u52_to_unit(x0: int, x1: int) -> float:
+    return float(lib().gpfc_ref_u52_to_unit(int(x0), int(x1)))
+
+
+def normal(seed: int, curve: int, i: int) -> float:
+    return float(lib().gpfc_ref_normal(int(seed), int(curve), int(i)))
+
+
+def make_light_curves(seed, ncurves, n, prm: LcParams, want_times=True):
+    """-> (times fp64 [ncurves][n] or None, flux fp32 [ncurves][n], params fp64 [ncurves][8])."""
+    times = np.empty((ncurves, n), np.float64) if want_times else None
+    flux = np.empty((ncurves, n), np.float32)
+    par = np.empty((ncurves, 8), np.float64)
+    _chk(lib().gpfc_ref_make_light_curves(int(seed), int(ncurves), int(n), ctypes.byref(prm),
+                                          _p(times), _p(flux), _p(par)),
+         "gpfc_ref_make_light_curves")
+    return times, flux, par
