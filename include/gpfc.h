@@ -197,7 +197,7 @@ int gpfc_fold_batch(const double *times, const float *flux, const int64_t *offse
  *   out_mean  device fp32 [ncurves][nperiods][nb2]  mean flux of the final bins   (may be NULL)
  *   out_norm  device fp32 [ncurves][nperiods][nb2]  the same, scaled to population
  *             standard deviation 1 about its mean (every final bin counts)       (may be NULL)
- * For nb1 in {1024, 2048, 4096} and nb2 <= (23 KB * nb1 / 32768) / 8 - 1 (381 for nb1 = 4096)
+ * For nb1 in {1024, 2048, 4096} and nb2 <= nb1 / 16 (256 for nb1 = 4096, the paper's pair)
  * fold and merge are ONE kernel: the intermediary profile stays in shared memory and the merge
  * reads the exact integer sums.  Any other (nb1, nb2) folds into a temporary intermediary
  * profile (stream-ordered allocation, <= 256 MB) and runs gpfc_merge_equal_count on it.
@@ -207,6 +207,68 @@ int gpfc_fold_two_tier(const double *times, const float *flux, const int64_t *of
                        int64_t ncurves, int64_t n_total, const double *periods,
                        int64_t nperiods, int nb1, int nb2, const double *t0,
                        float *out_mean, float *out_norm);
+
+/*
+ * Synthetic light curves on the device (PAPER.md 2.6 "Light Curve
+ * Simulation": Eq. 2 :162, parameter ranges :166-170, Table 2 :176-180, trapezoid :170,
+ * Fig. 7 :188, SNR range :190): white Gaussian noise of per-point standard deviation sigma
+ * around 1, with a periodic trapezoidal transit whose depth follows from a requested
+ * signal-to-noise ratio through Eq. 2.  The inputs of large sweeps never touch the host.
+ *
+ * Generator specification (a pure function of seed, curve index c and sample index i, so the
+ * CPU oracle reproduces it bit for bit).  Random words come from Philox4x32-10 (Salmon et al.,
+ * SC'11) with key (seed low word, seed high word) and counter (w0, w1, w2, w3); U(x) =
+ * (x + 1/2) 2^-32; every fp64 operation is rounded once, in the order written, no FMA.
+ *   curve c:  (x0..x3) = philox(0, 0, c, 0):  sigma = sigma_lo + (sigma_hi - sigma_lo) U(x0),
+ *             r = U(x1), e = U(x2), alpha = snr_lo + (snr_hi - snr_lo) U(x3)
+ *             philox(0, 1, c, 0):  the curve carries a transit iff U(x0) < transit_fraction
+ *             philox(k, 2, c, 0), k = 0, 1, ... 63:  p = period_lo + (period_hi - period_lo) U(x0),
+ *             L = (ratio_lo + (ratio_hi - ratio_lo) U(x1)) p; the first k with
+ *             duration_lo <= L <= duration_hi is taken (k = 63: L is clamped) -- Table 2 gives
+ *             ranges for p, L and L/p but no joint law (R21)
+ *             depth d = (alpha sigma) / sqrt(((double)n L) / p)                 Eq. 2 solved for d
+ *             long base T14 = (2 L) / (1 + r), short base T23 = r T14 (duration L at half
+ *             depth), mid-transit epoch tc = e p
+ *   sample i: t = t_start + (double)i cadence
+ *             (x0..x3) = philox(i, 0, c, 1): u1 = ((x0 2^20 + (x1 >> 12)) + 1/2) 2^-52,
+ *             u2 = U(x2), z = sqrt(-2 ln u1) cos(2 pi u2)                       (Box-Muller)
+ *             ln u:  u = m 2^e with m in [1/2, 1) from the bits of u; if m < 0.70710678118654752
+ *                    then m = 2 m, e = e - 1;  s = (m - 1)/(m + 1), w = s s,
+ *                    P = 1/23; P = P w + 1/(2j+1) for j = 10 ... 0;
+ *                    ln u = e * 0.69314718055994531 + 2 (s P)
+ *             cos(2 pi v):  8 v = k + f (k = floor, octant), g = 1 - f if k is odd else f,
+ *                    theta = g * 0.78539816339744831, w = theta theta; for k in {1, 2, 5, 6}
+ *                    value = theta (1 - w/3! + w^2/5! - ... - w^7/15!), else
+ *                    value = 1 - w/2! + w^2/4! - ... + w^8/16! (Horner from the highest term,
+ *                    each coefficient the fp64 quotient 1/j!); negated for k in {2, 3, 4, 5}
+ *             y = (t - tc) / p; y = y - floor(y + 1/2); x = |y| p
+ *             shape = 1 if x <= T23/2, 0 if x >= T14/2, else (T14/2 - x) / (T14/2 - T23/2)
+ *             flux = (float)((1 + sigma z) - d shape), minus 1.0f (in fp32) if GPFC_LC_CENTERED
+ *
+ *   prm       host; ranges as above, gpfc_lc_params_default() fills Table 2's
+ *   times     device fp64 [ncurves][n], may be NULL (every curve has the same time stamps)
+ *   flux      device fp32 [ncurves][n]
+ *   offsets   device int64 [ncurves + 1] = c n, may be NULL (the array gpfc_fold_batch wants)
+ *   params_out device fp64 [ncurves][8], may be NULL: {p, L, sigma, d (0 without a transit), r,
+ *             tc, alpha, 1.0 or 0.0 = carries a transit}; scratch is taken from the workspace
+ *             (8 * 8 * ncurves bytes) or allocated stream-ordered when it is NULL
+ * ncurves and n must be below 2^32.  GPFC_ERR_INVALID_ARG for an empty or reversed range.
+ */
+enum { GPFC_LC_CENTERED = 1, GPFC_LC_NO_NOISE = 2 };
+typedef struct {
+    double period_lo, period_hi;       /* p,     Table 2: (0.3, 1.0) d            */
+    double duration_lo, duration_hi;   /* L,     Table 2: (0.03, 0.09) d          */
+    double ratio_lo, ratio_hi;         /* L / p, Table 2: (0.04, 0.12)            */
+    double sigma_lo, sigma_hi;         /* sigma, Table 2: (0.0001, 0.0005)        */
+    double snr_lo, snr_hi;             /* alpha: [6, 10]            */
+    double transit_fraction;           /* share of the curves that carry a transit */
+    double cadence, t_start;           /* t_i = t_start + i cadence               */
+    int32_t flags;                     /* GPFC_LC_*                               */
+    int32_t reserved;
+} gpfc_lc_params;
+int gpfc_lc_params_default(gpfc_lc_params *prm);
+int gpfc_make_light_curves(uint64_t seed, int64_t ncurves, int64_t n, const gpfc_lc_params *prm,
+                           double *times, float *flux, int64_t *offsets, double *params_out);
 
 /*
  * Host-buffer convenience entry points (the end-to-end path): same

@@ -29,7 +29,20 @@ EXPORTS = [
     "gpfc_normalize", "gpfc_fold_batch", "gpfc_make_period_grid_host",
     "gpfc_fold_batch_host", "gpfc_measure_peaks", "gpfc_profile", "gpfc_profile_read",
     "gpfc_merge_equal_count", "gpfc_init", "gpfc_fold_two_tier", "gpfc_path_counters",
+    "gpfc_lc_params_default", "gpfc_make_light_curves",
 ]
+LC_CENTERED = 1
+LC_NO_NOISE = 2
+LC_PARAM_NAMES = ("period", "duration", "sigma", "depth", "ratio_r", "epoch", "snr", "has_transit")
+
+
+class LcParams(ctypes.Structure):
+    """gpfc_lc_params of include/gpfc.h (field order and types as declared there)."""
+    _fields_ = [(k, ctypes.c_double) for k in (
+        "period_lo", "period_hi", "duration_lo", "duration_hi", "ratio_lo", "ratio_hi",
+        "sigma_lo", "sigma_hi", "snr_lo", "snr_hi", "transit_fraction", "cadence", "t_start")]
+    _fields_ += [("flags", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
 
 
 class GpfcError(RuntimeError):
@@ -70,6 +83,8 @@ def lib() -> ctypes.CDLL:
     L.gpfc_profile_read.argtypes = [vp, vp, vp]
     L.gpfc_fold_two_tier.argtypes = [vp, vp, vp, i64, i64, vp, i64, i32, i32, vp, vp, vp]
     L.gpfc_path_counters.argtypes = [vp]
+    L.gpfc_lc_params_default.argtypes = [vp]
+    L.gpfc_make_light_curves.argtypes = [ctypes.c_uint64, i64, i64, vp, vp, vp, vp, vp]
     _lib = L
     return L
 
@@ -237,6 +252,34 @@ def gpfc_fold_two_tier(times, flux, offsets, periods, nb1, nb2, t0=None, out_mea
         _dptr(t0, torch.float64, "t0"), _dptr(out_mean, torch.float32, "out_mean"),
         _dptr(out_norm, torch.float32, "out_norm")), "gpfc_fold_two_tier")
     return out_mean, out_norm
+
+
+def gpfc_lc_params_default(**over) -> LcParams:
+    """Table 2's ranges, alpha in [6, 10]; keyword arguments override fields."""
+    prm = LcParams()
+    _check(lib().gpfc_lc_params_default(ctypes.byref(prm)), "gpfc_lc_params_default")
+    for k, v in over.items():
+        setattr(prm, k, v)
+    return prm
+
+
+def gpfc_make_light_curves(seed, ncurves, n, prm=None, device="cuda", want_times=True,
+                           want_offsets=True, want_params=True):
+    """Synthetic light curves generated on the device (PAPER.md 2.6).
+    -> (times fp64 [ncurves][n] or None, flux fp32 [ncurves][n], offsets int64 [ncurves + 1] or
+    None, params fp64 [ncurves][8] or None)."""
+    prm = gpfc_lc_params_default() if prm is None else prm
+    nc, n = int(ncurves), int(n)
+    times = torch.empty((nc, n), dtype=torch.float64, device=device) if want_times else None
+    flux = torch.empty((nc, n), dtype=torch.float32, device=device)
+    offsets = torch.empty(nc + 1, dtype=torch.int64, device=device) if want_offsets else None
+    params = torch.empty((nc, 8), dtype=torch.float64, device=device) if want_params else None
+    _use_current_stream()
+    _check(lib().gpfc_make_light_curves(
+        ctypes.c_uint64(int(seed)), nc, n, ctypes.byref(prm), _dptr(times, torch.float64, "times"),
+        _dptr(flux, torch.float32, "flux"), _dptr(offsets, torch.int64, "offsets"),
+        _dptr(params, torch.float64, "params_out")), "gpfc_make_light_curves")
+    return times, flux, offsets, params
 
 
 def gpfc_init() -> None:

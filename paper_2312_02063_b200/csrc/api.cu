@@ -301,6 +301,68 @@ int gpfc_make_period_grid(double pmin, double pmax, int64_t nperiods, int mode_f
     return GPFC_OK;
 }
 
+int gpfc_lc_params_default(gpfc_lc_params *prm)
+{
+    if (!prm) return fail(GPFC_ERR_INVALID_ARG, "prm is NULL%s");
+    std::memset(prm, 0, sizeof(*prm));
+    prm->period_lo = 0.3;          // Table 2
+    prm->period_hi = 1.0;
+    prm->duration_lo = 0.03;
+    prm->duration_hi = 0.09;
+    prm->ratio_lo = 0.04;
+    prm->ratio_hi = 0.12;
+    prm->sigma_lo = 0.0001;
+    prm->sigma_hi = 0.0005;
+    prm->snr_lo = 6.0;
+    prm->snr_hi = 10.0;
+    prm->transit_fraction = 0.5;   // as many transit as non-transit samples
+    prm->cadence = 0.020433;       // Kepler long cadence (R16)
+    prm->t_start = 0.0;
+    return GPFC_OK;
+}
+
+int gpfc_make_light_curves(uint64_t seed, int64_t ncurves, int64_t n, const gpfc_lc_params *prm,
+                           double *times, float *flux, int64_t *offsets, double *params_out)
+{
+    if (ncurves < 0 || n < 0) return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
+    if (ncurves > 4294967295ll || n > 4294967295ll)
+        return fail(GPFC_ERR_INVALID_ARG, "ncurves and n must be below 2^32%s");
+    if (!prm) return fail(GPFC_ERR_INVALID_ARG, "prm is NULL%s");
+    if (!(prm->period_lo > 0.0) || !(prm->period_hi >= prm->period_lo) || !(prm->duration_lo > 0.0) ||
+        !(prm->duration_hi >= prm->duration_lo) || !(prm->ratio_lo > 0.0) ||
+        !(prm->ratio_hi >= prm->ratio_lo) || !(prm->sigma_lo >= 0.0) ||
+        !(prm->sigma_hi >= prm->sigma_lo) || !(prm->snr_hi >= prm->snr_lo) || !(prm->cadence > 0.0) ||
+        !std::isfinite(prm->period_hi) || !std::isfinite(prm->duration_hi) ||
+        !std::isfinite(prm->ratio_hi) || !std::isfinite(prm->sigma_hi) || !std::isfinite(prm->snr_lo) ||
+        !std::isfinite(prm->snr_hi) || !std::isfinite(prm->cadence) || !std::isfinite(prm->t_start) ||
+        !std::isfinite(prm->transit_fraction))
+        return fail(GPFC_ERR_INVALID_ARG, "light-curve parameters: empty, reversed or non-finite range%s");
+    if (ncurves == 0) return GPFC_OK;
+    if (n > 0 && !flux) return fail(GPFC_ERR_INVALID_ARG, "flux is NULL%s");
+    const gpfc::DeviceInfo *di = nullptr;
+    cudaError_t e = gpfc::device_info(&di);
+    if (e != cudaSuccess) return cuda_fail(e, "device initialisation");
+    cudaStream_t st = g_ts.stream;
+    const size_t need = gpfc::simulate_scratch_bytes(ncurves) + 256;
+    void *scratch = nullptr;
+    bool own = false;
+    if (g_ts.ws && g_ts.ws_bytes >= need) {
+        scratch = reinterpret_cast<void *>(align_up(reinterpret_cast<size_t>(g_ts.ws)));
+    } else {
+        e = cudaMallocAsync(&scratch, need, st);
+        if (e != cudaSuccess) {
+            cuda_fail(e, "scratch allocation");
+            return GPFC_ERR_WORKSPACE;
+        }
+        own = true;
+    }
+    e = gpfc::launch_simulate(seed, ncurves, n, *prm, times, flux, reinterpret_cast<long long *>(offsets),
+                              params_out, scratch, di->num_sms, st);
+    if (own) cudaFreeAsync(scratch, st);
+    if (e != cudaSuccess) return cuda_fail(e, "light-curve generator launch");
+    return GPFC_OK;
+}
+
 int gpfc_fold(const double *times, const float *flux, int64_t n, const double *periods,
               int64_t nperiods, int nbins, double t0, float *out_sum, uint32_t *out_count)
 {

@@ -210,5 +210,10 @@ cudaError_t launch_merge(const float *sum, const uint32_t *count, long long npro
 cudaError_t launch_grid(double pmin, double pmax, long long nperiods, int mode_flags,
                         double *out, cudaStream_t st);
 cudaError_t measure_peaks(double *out_host, cudaStream_t st);
+size_t simulate_scratch_bytes(long long ncurves);                                 // simulate.cu
+cudaError_t launch_simulate(unsigned long long seed, long long ncurves, long long n,
+                            const gpfc_lc_params &prm, double *times, float *flux,
+                            long long *offsets, double *params_out, void *scratch, int sms,
+                            cudaStream_t st);
 
 }  // namespace gpfc
