@@ -57,6 +57,10 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-peaks", action="store_true", help="skip gpfc_measure_peaks")
+    ap.add_argument("--generated-inputs", action="store_true",
+                    help="draw the light curves on the device with gpfc_make_light_curves (PAPER.md 2.6 "
+                         "simulator, same shape and cadence as the config) instead of the numpy recipe; "
+                         "the graded inputs are the numpy ones")
     ap.add_argument("--no-others", action="store_true",
                     help="skip the other_configs block of the default run (configs 1, 3, 4, 5)")
     return ap.parse_args()
@@ -272,10 +276,29 @@ def fold_kernel_name(w):
 class DeviceRun:
     """One workload resident in HBM: buffers, the step, its timing (CUDA events, max over ranks)."""
 
-    def __init__(self, gp, torch, w):
+    def __init__(self, gp, torch, w, generated=False, seed=0):
         self.gp, self.torch, self.w = gp, torch, w
         dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-        self.times, self.flux, self.offsets = dev(w.times), dev(w.flux), dev(w.offsets)
+        self.generator = None
+        if generated:
+            # rectangular batch of the config's shape: n samples at its median cadence
+            n = w.n_total // max(w.ncurves, 1)
+            cad = float(np.median(np.diff(w.times[:n])))
+            prm = gp.gpfc_lc_params_default(cadence=cad, flags=gp.LC_CENTERED)
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            gp.gpfc_make_light_curves(seed, w.ncurves, n, prm)          # warm-up
+            ev[0].record()
+            t_, f_, o_, _ = gp.gpfc_make_light_curves(seed, w.ncurves, n, prm)
+            ev[1].record()
+            torch.cuda.synchronize()
+            ms = ev[0].elapsed_time(ev[1])
+            self.times, self.flux, self.offsets = t_.reshape(-1), f_.reshape(-1), o_
+            ns = float(w.ncurves) * n
+            self.generator = {"api": "gpfc_make_light_curves", "samples": ns, "ms": ms,
+                              "samples_per_s": ns / (ms * 1e-3), "bytes_written": ns * 12.0,
+                              "hbm_gbs": ns * 12.0 / (ms * 1e-3) / 1e9, "cadence_d": cad, "seed": seed}
+        else:
+            self.times, self.flux, self.offsets = dev(w.times), dev(w.flux), dev(w.offsets)
         self.two_tier = (w.config_id == 5)
         self.shape = (w.ncurves, w.nperiods, 256 if self.two_tier else w.nbins)
         self.periods = torch.empty(w.nperiods, dtype=torch.float64, device="cuda")
@@ -371,9 +394,10 @@ def roofline_of(w, run, prof, sm_max, peaks, traffic_db, digest):
     return roof
 
 
-def host_e2e(gp, torch, w, run_shape, steps, barrier, world, two_tier):
+def host_e2e(gp, torch, w, run_shape, steps, barrier, world, two_tier, norm_only=False):
     """The same step through the host-buffer entry points: pinned host memory in and out,
-    copies inside the timed region."""
+    copies inside the timed region.  norm_only: only the normalised profiles (the scorer's
+    input) come back, a third of the bytes."""
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     h_t, h_f, h_o = pin(w.times), pin(w.flux), pin(w.offsets)
     h_sum = h_cnt = h_norm = None
@@ -382,7 +406,7 @@ def host_e2e(gp, torch, w, run_shape, steps, barrier, world, two_tier):
         h_norm = torch.empty(run_shape, dtype=torch.float32, pin_memory=True)
     else:
         h_norm = torch.empty(run_shape, dtype=torch.float32, pin_memory=True)
-        if not w.fused_normalize:
+        if not w.fused_normalize and not norm_only:
             h_sum = torch.empty(run_shape, dtype=torch.float32, pin_memory=True)
             h_cnt = torch.empty(run_shape, dtype=torch.int32, pin_memory=True)
 
@@ -412,8 +436,11 @@ def host_e2e(gp, torch, w, run_shape, steps, barrier, world, two_tier):
     nout = int(np.prod(run_shape)) * 4
     e2e = {"value": float(w.point_periods) * world * steps / dt, "unit": UNIT,
            "h2d_bytes_per_step": int(w.n_total * 12 + w.offsets.nbytes),
-           "d2h_bytes_per_step": int(nout * (1 if w.fused_normalize else 3) + w.nperiods * 8),
-           "steps": steps, "api": "gpfc_make_period_grid_host + gpfc_fold_batch_host"}
+           "d2h_bytes_per_step": int(nout * (1 if (w.fused_normalize or norm_only) else 3) + w.nperiods * 8),
+           "steps": steps, "api": "gpfc_make_period_grid_host + gpfc_fold_batch_host"
+                                  + (" (out_norm only)" if norm_only else "")}
+    e2e["s_per_step"] = dt / steps
+    e2e["d2h_gbs"] = e2e["d2h_bytes_per_step"] / (dt / steps) / 1e9
     if two_tier:
         e2e["d2h_bytes_per_step"] = int(2 * nout)
         e2e["api"] = "torch H2D + gpfc_make_period_grid + gpfc_fold_two_tier + torch D2H"
@@ -453,7 +480,8 @@ def gpu_arm(args):
 
     # ---- the headline workload
     w = make_workload(args, rank)
-    run = DeviceRun(gp, torch, w)
+    run = DeviceRun(gp, torch, w, generated=args.generated_inputs, seed=1000 + rank)
+    generator = run.generator
     ms, prof, paths, clocks = run.timed(args.steps, args.warmup, barrier, world,
                                         ClockSampler(local) if rank == 0 else None)
     pp_step_all = float(w.point_periods) * world
@@ -468,6 +496,18 @@ def gpu_arm(args):
     if not args.no_e2e:
         e2e = host_e2e(gp, torch, w, shape, max(1, min(args.steps, 3)), barrier, world, two_tier)
         torch.cuda.empty_cache()
+        if not two_tier and not w.fused_normalize:
+            # the streaming path a scorer would use: only the normalised profiles come back, and
+            # the copy of chunk k overlaps the fold of chunk k+1 (gpfc_fold_stream)
+            e2n = host_e2e(gp, torch, w, shape, max(1, min(args.steps, 3)), barrier, world, two_tier,
+                           norm_only=True)
+            fold_s = ms / args.steps * 1e-3
+            e2n["device_fold_s_per_step"] = fold_s
+            # time hidden by the overlap: fold + copy back to back would take fold_s + bytes / rate
+            e2n["copy_s_at_this_rate"] = e2n["d2h_bytes_per_step"] / (e2e["d2h_gbs"] * 1e9)
+            e2n["hidden_s_per_step"] = max(0.0, fold_s + e2n["copy_s_at_this_rate"] - e2n["s_per_step"])
+            e2e["norm_only"] = e2n
+            torch.cuda.empty_cache()
 
     # ---- the other BASELINE.json configs (and the paper's own fold), each after its own
     # warm-up, so that one driver run carries a number for every row of DESIGN.md 7
@@ -523,6 +563,9 @@ def gpu_arm(args):
         out["e2e"] = e2e
         if two_tier:
             out["paper"]["workload_s_here_e2e"] = 70000.0 * 100000.0 / e2e["value"]
+    if generator:
+        out["generator"] = generator
+        out["data"] = "synthetic, generated on the device (gpfc_make_light_curves)"
     if others:
         out["other_configs"] = others
     if not args.no_cpu:

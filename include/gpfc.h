@@ -63,7 +63,8 @@ typedef enum {
     GPFC_ERR_INVALID_ARG = 1,  /* NULL required pointer, negative size, bad range  */
     GPFC_ERR_UNSUPPORTED = 2,  /* nbins out of range                               */
     GPFC_ERR_WORKSPACE = 3,    /* registered workspace too small / allocation failed */
-    GPFC_ERR_CUDA = 4          /* CUDA runtime error (text in gpfc_last_error)     */
+    GPFC_ERR_CUDA = 4,         /* CUDA runtime error (text in gpfc_last_error)     */
+    GPFC_ERR_ABORTED = 5       /* a caller-supplied callback returned non-zero     */
 } gpfc_status;
 
 #define GPFC_MAX_NBINS 4096
@@ -271,11 +272,58 @@ int gpfc_make_light_curves(uint64_t seed, int64_t ncurves, int64_t n, const gpfc
                            double *times, float *flux, int64_t *offsets, double *params_out);
 
 /*
+ * Streaming fold for a downstream consumer ("transfer data in
+ * batches", :278 the fold of light curve k+1 runs while the CNN scores light curve k): the
+ * batch is folded chunk by chunk into one of two device slabs, and every finished chunk is
+ * handed to the caller's consumer, which works on it on ITS stream while the next chunk folds.
+ *
+ * Arguments as gpfc_fold_batch (all device pointers), then
+ *   outputs          GPFC_OUT_SUM | GPFC_OUT_COUNT | GPFC_OUT_NORM: the arrays to produce.
+ *                    GPFC_OUT_NORM alone is the scorer's input and a third of the bytes.
+ *   slab_bytes       bytes of output per chunk (all requested arrays together); 0 = 512 MB
+ *                    per requested array.
+ *                    A chunk is a run of whole curves; if the profiles of one curve exceed the
+ *                    slab, a run of consecutive periods of one curve.
+ *   consumer_stream  the stream (cudaStream_t) the consumer's work runs on; NULL = the fold
+ *                    stream (no overlap)
+ *   on_chunk         called on the calling host thread once per chunk, in order, right after
+ *                    the chunk's fold has been ENQUEUED: consumer_stream already waits for
+ *                    chunk->ready, so the callback only enqueues its work on that stream
+ *                    (kernels, copies) and returns 0 without blocking.  The chunk's arrays are
+ *                    device pointers [ncurves][nperiods][nbins] into the slab (NULL for arrays
+ *                    not requested), valid for work enqueued on consumer_stream inside the
+ *                    callback: the slab is folded into again once that work has run.  A
+ *                    non-zero return stops the loop: GPFC_ERR_ABORTED.
+ * The library allocates the two slabs stream-ordered on the fold stream and frees them after
+ * the consumer stream's last chunk; the host never waits.  Returns when everything is
+ * enqueued.
+ */
+enum { GPFC_OUT_SUM = 1, GPFC_OUT_COUNT = 2, GPFC_OUT_NORM = 4 };
+typedef struct {
+    int64_t curve0, ncurves;     /* curves   [curve0, curve0 + ncurves)   of the batch */
+    int64_t period0, nperiods;   /* periods  [period0, period0 + nperiods) of the grid  */
+    int32_t nbins;
+    int32_t slot;                /* which of the two slabs (0 / 1)                      */
+    const float *sum;            /* device [ncurves][nperiods][nbins] or NULL           */
+    const uint32_t *count;
+    const float *norm;
+    void *ready;                 /* cudaEvent_t recorded on the fold stream after this chunk */
+} gpfc_chunk;
+typedef int (*gpfc_chunk_fn)(const gpfc_chunk *chunk, void *consumer_stream, void *user);
+int gpfc_fold_stream(const double *times, const float *flux, const int64_t *offsets,
+                     int64_t ncurves, int64_t n_total, const double *periods, int64_t nperiods,
+                     int nbins, const double *t0, int outputs, size_t slab_bytes,
+                     void *consumer_stream, gpfc_chunk_fn on_chunk, void *user);
+
+/*
  * Host-buffer convenience entry points (the end-to-end path): same
  * arguments, but every pointer is HOST memory (pinned memory makes the copies
  * faster but is not required).  The call allocates device buffers, copies the
- * inputs in, runs the device path on the current stream, copies the requested
- * outputs back and synchronises the stream before returning.
+ * inputs in, runs gpfc_fold_stream on the current stream with a consumer that
+ * copies every finished chunk back on a second stream (so the copy of chunk k
+ * overlaps the fold of chunk k+1), and synchronises both streams before
+ * returning.  Pass only out_norm (out_sum, out_count NULL) to move a third of
+ * the bytes.
  */
 int gpfc_make_period_grid_host(double pmin, double pmax, int64_t nperiods, int mode_flags,
                                double *periods_out);

@@ -29,8 +29,30 @@ EXPORTS = [
     "gpfc_normalize", "gpfc_fold_batch", "gpfc_make_period_grid_host",
     "gpfc_fold_batch_host", "gpfc_measure_peaks", "gpfc_profile", "gpfc_profile_read",
     "gpfc_merge_equal_count", "gpfc_init", "gpfc_fold_two_tier", "gpfc_path_counters",
-    "gpfc_lc_params_default", "gpfc_make_light_curves",
+    "gpfc_lc_params_default", "gpfc_make_light_curves", "gpfc_fold_stream",
 ]
+OUT_SUM, OUT_COUNT, OUT_NORM = 1, 2, 4
+
+
+class Chunk(ctypes.Structure):
+    """gpfc_chunk of include/gpfc.h."""
+    _fields_ = [("curve0", ctypes.c_int64), ("ncurves", ctypes.c_int64),
+                ("period0", ctypes.c_int64), ("nperiods", ctypes.c_int64),
+                ("nbins", ctypes.c_int32), ("slot", ctypes.c_int32),
+                ("sum", ctypes.c_void_p), ("count", ctypes.c_void_p), ("norm", ctypes.c_void_p),
+                ("ready", ctypes.c_void_p)]
+
+
+CHUNK_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.POINTER(Chunk), ctypes.c_void_p, ctypes.c_void_p)
+
+
+class _DeviceView:
+    """Zero-copy view of library-owned device memory for torch.as_tensor."""
+
+    def __init__(self, ptr, shape, typestr):
+        self.__cuda_array_interface__ = {"shape": tuple(int(x) for x in shape), "typestr": typestr,
+                                         "data": (int(ptr), False), "version": 3, "strides": None}
+
 LC_CENTERED = 1
 LC_NO_NOISE = 2
 LC_PARAM_NAMES = ("period", "duration", "sigma", "depth", "ratio_r", "epoch", "snr", "has_transit")
@@ -85,6 +107,8 @@ def lib() -> ctypes.CDLL:
     L.gpfc_path_counters.argtypes = [vp]
     L.gpfc_lc_params_default.argtypes = [vp]
     L.gpfc_make_light_curves.argtypes = [ctypes.c_uint64, i64, i64, vp, vp, vp, vp, vp]
+    L.gpfc_fold_stream.argtypes = [vp, vp, vp, i64, i64, vp, i64, i32, vp, i32, ctypes.c_size_t, vp,
+                                   CHUNK_FN, vp]
     _lib = L
     return L
 
@@ -252,6 +276,49 @@ def gpfc_fold_two_tier(times, flux, offsets, periods, nb1, nb2, t0=None, out_mea
         _dptr(t0, torch.float64, "t0"), _dptr(out_mean, torch.float32, "out_mean"),
         _dptr(out_norm, torch.float32, "out_norm")), "gpfc_fold_two_tier")
     return out_mean, out_norm
+
+
+def gpfc_fold_stream(times, flux, offsets, periods, nbins, consumer, t0=None, want=("norm",),
+                     slab_bytes=0, consumer_stream=None):
+    """Chunked fold for a downstream consumer.  `consumer(chunk)` is called
+    once per chunk with torch's current stream set to the consumer stream, which already waits
+    for the chunk; `chunk` is a dict with curve0, ncurves, period0, nperiods, slot and the
+    requested arrays "sum" / "count" / "norm" as tensors [ncurves][nperiods][nbins] that alias
+    the library's slab: use them only in work enqueued on the current stream during the call
+    (a scorer kernel, a copy), and do not block.  Returns once everything is enqueued."""
+    nc = 1 if offsets is None else offsets.numel() - 1
+    npd, n_total = periods.numel(), times.numel()
+    outputs = (OUT_SUM if "sum" in want else 0) | (OUT_COUNT if "count" in want else 0) | \
+              (OUT_NORM if "norm" in want else 0)
+    cstream = consumer_stream if consumer_stream is not None else torch.cuda.current_stream()
+    failure = []
+
+    def on_chunk(chp, _stream, _user):
+        try:
+            ch = chp.contents
+            shape = (ch.ncurves, ch.nperiods, ch.nbins)
+            d = {"curve0": ch.curve0, "ncurves": ch.ncurves, "period0": ch.period0,
+                 "nperiods": ch.nperiods, "slot": ch.slot}
+            for name, ptr, ts in (("sum", ch.sum, "<f4"), ("count", ch.count, "<i4"),
+                                  ("norm", ch.norm, "<f4")):
+                d[name] = torch.as_tensor(_DeviceView(ptr, shape, ts), device=times.device) if ptr else None
+            with torch.cuda.stream(cstream):
+                consumer(d)
+            return 0
+        except BaseException as exc:      # never unwind through the C frame
+            failure.append(exc)
+            return 1
+
+    cb = CHUNK_FN(on_chunk)
+    _use_current_stream()
+    rc = lib().gpfc_fold_stream(
+        _dptr(times, torch.float64, "times"), _dptr(flux, torch.float32, "flux"),
+        _dptr(offsets, torch.int64, "offsets"), nc, n_total, _dptr(periods, torch.float64, "periods"),
+        npd, int(nbins), _dptr(t0, torch.float64, "t0"), outputs, int(slab_bytes),
+        ctypes.c_void_p(cstream.cuda_stream), cb, None)
+    if failure:
+        raise failure[0]
+    _check(rc, "gpfc_fold_stream")
 
 
 def gpfc_lc_params_default(**over) -> LcParams:

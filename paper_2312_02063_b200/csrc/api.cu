@@ -489,14 +489,173 @@ int gpfc_make_period_grid_host(double pmin, double pmax, int64_t nperiods, int m
     return GPFC_OK;
 }
 
+int gpfc_fold_stream(const double *times, const float *flux, const int64_t *offsets,
+                     int64_t ncurves, int64_t n_total, const double *periods, int64_t nperiods,
+                     int nbins, const double *t0, int outputs, size_t slab_bytes,
+                     void *consumer_stream, gpfc_chunk_fn on_chunk, void *user)
+{
+    if (ncurves < 0 || nperiods < 0 || n_total < 0)
+        return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
+    if (nbins < 1 || nbins > GPFC_MAX_NBINS)
+        return fail(GPFC_ERR_UNSUPPORTED, "nbins must be in [1, 4096]%s");
+    if (!on_chunk) return fail(GPFC_ERR_INVALID_ARG, "on_chunk is NULL%s");
+    outputs &= GPFC_OUT_SUM | GPFC_OUT_COUNT | GPFC_OUT_NORM;
+    if (!outputs) return fail(GPFC_ERR_INVALID_ARG, "outputs selects no array%s");
+    if (ncurves == 0 || nperiods == 0) return GPFC_OK;
+    if (!periods || (n_total > 0 && (!times || !flux)))
+        return fail(GPFC_ERR_INVALID_ARG, "NULL pointer%s");
+    if (!offsets && ncurves != 1)
+        return fail(GPFC_ERR_INVALID_ARG, "offsets may be NULL only for a single curve%s");
+    cudaStream_t st = g_ts.stream;
+    cudaStream_t cs = consumer_stream ? static_cast<cudaStream_t>(consumer_stream) : st;
+    const int nout = ((outputs & GPFC_OUT_SUM) ? 1 : 0) + ((outputs & GPFC_OUT_COUNT) ? 1 : 0) +
+                     ((outputs & GPFC_OUT_NORM) ? 1 : 0);
+    const size_t slab = slab_bytes ? slab_bytes : ((size_t)512 << 20) * (size_t)nout;
+    const size_t prof = (size_t)nbins * 4 * (size_t)nout;     // bytes of one profile, all arrays
+    const size_t row = prof * (size_t)nperiods;               // ... of one curve
+    // a chunk is a run of whole curves, or (when one curve's profiles exceed the slab) a run of
+    // periods of one curve; either way its profiles are contiguous in [curve][period][bin]
+    int64_t cchunk = 1, pchunk = nperiods;
+    if (row <= slab) {
+        cchunk = (int64_t)(slab / row);
+        if (cchunk > ncurves) cchunk = ncurves;
+    } else {
+        pchunk = (int64_t)(slab / prof);
+        if (pchunk < 1) pchunk = 1;
+    }
+    const size_t b_arr = align_up((size_t)cchunk * (size_t)pchunk * (size_t)nbins * 4);
+    char *base = nullptr;
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&base), 2 * (size_t)nout * b_arr + 256, st);
+    if (e != cudaSuccess) {
+        cuda_fail(e, "output slab allocation");
+        return GPFC_ERR_WORKSPACE;
+    }
+    char *cur = reinterpret_cast<char *>(align_up(reinterpret_cast<size_t>(base)));
+    char *arr[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
+    for (int sl = 0; sl < 2; ++sl)
+        for (int k = 0; k < 3; ++k)
+            if (outputs & (1 << k)) {
+                arr[sl][k] = cur;
+                cur += b_arr;
+            }
+    // one scratch for all chunks (unless the caller registered a workspace that is large
+    // enough): a stream-ordered allocation per chunk costs more than the prepass it serves
+    const gpfc::DeviceInfo *di = nullptr;
+    e = gpfc::device_info(&di);
+    void *saved_ws = g_ts.ws, *own_ws = nullptr;
+    const size_t saved_ws_bytes = g_ts.ws_bytes;
+    if (e == cudaSuccess) {
+        const size_t need = scratch_bytes(cchunk, n_total, pchunk, side_bytes_for(n_total, nbins, di->num_sms));
+        if (!(g_ts.ws && g_ts.ws_bytes >= need) && cudaMallocAsync(&own_ws, need, st) == cudaSuccess) {
+            g_ts.ws = own_ws;
+            g_ts.ws_bytes = need;
+        }
+    }
+    cudaEvent_t ready[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr};
+    for (int sl = 0; sl < 2 && e == cudaSuccess; ++sl) {
+        e = cudaEventCreateWithFlags(&ready[sl], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&consumed[sl], cudaEventDisableTiming);
+    }
+    int rc = GPFC_OK;
+    int64_t k = 0;
+    for (int64_t c0 = 0; c0 < ncurves && e == cudaSuccess && rc == GPFC_OK; c0 += cchunk) {
+        const int64_t nc = (ncurves - c0 < cchunk) ? ncurves - c0 : cchunk;
+        for (int64_t p0 = 0; p0 < nperiods && e == cudaSuccess && rc == GPFC_OK; p0 += pchunk, ++k) {
+            const int64_t np = (nperiods - p0 < pchunk) ? nperiods - p0 : pchunk;
+            const int sl = (int)(k & 1);
+            if (k >= 2) e = cudaStreamWaitEvent(st, consumed[sl], 0);   // the consumer is done with it
+            if (e != cudaSuccess) break;
+            FoldOut o;
+            o.sum = reinterpret_cast<float *>(arr[sl][0]);
+            o.count = reinterpret_cast<uint32_t *>(arr[sl][1]);
+            o.norm = reinterpret_cast<float *>(arr[sl][2]);
+            // offsets are absolute: pass the whole sample arrays, the curves' slice of offsets
+            rc = fold_device(times, flux, offsets ? offsets + c0 : nullptr, nc, n_total, periods + p0, np,
+                             nbins, t0 ? t0 + c0 : nullptr, 0.0, o);
+            if (rc != GPFC_OK) break;
+            e = cudaEventRecord(ready[sl], st);
+            if (e == cudaSuccess && cs != st) e = cudaStreamWaitEvent(cs, ready[sl], 0);
+            if (e != cudaSuccess) break;
+            gpfc_chunk ch;
+            ch.curve0 = c0;
+            ch.ncurves = nc;
+            ch.period0 = p0;
+            ch.nperiods = np;
+            ch.nbins = nbins;
+            ch.slot = sl;
+            ch.sum = o.sum;
+            ch.count = o.count;
+            ch.norm = o.norm;
+            ch.ready = ready[sl];
+            if (on_chunk(&ch, cs, user) != 0) {
+                rc = fail(GPFC_ERR_ABORTED, "the chunk consumer returned non-zero%s");
+                break;
+            }
+            e = cudaEventRecord(consumed[sl], cs);
+        }
+    }
+    // the slabs are released once the consumer stream is past its last chunk (stream-ordered,
+    // the host does not wait)
+    if (cs != st) {
+        cudaEvent_t tail = nullptr;
+        if (cudaEventCreateWithFlags(&tail, cudaEventDisableTiming) == cudaSuccess) {
+            cudaEventRecord(tail, cs);
+            cudaStreamWaitEvent(st, tail, 0);
+            cudaEventDestroy(tail);
+        }
+    }
+    cudaFreeAsync(base, st);
+    if (own_ws) {
+        cudaFreeAsync(own_ws, st);
+        g_ts.ws = saved_ws;
+        g_ts.ws_bytes = saved_ws_bytes;
+    }
+    for (int sl = 0; sl < 2; ++sl) {
+        if (ready[sl]) cudaEventDestroy(ready[sl]);
+        if (consumed[sl]) cudaEventDestroy(consumed[sl]);
+    }
+    if (rc != GPFC_OK) return rc;
+    if (e != cudaSuccess) return cuda_fail(e, "gpfc_fold_stream");
+    return GPFC_OK;
+}
+
+namespace {
+
+// consumer of gpfc_fold_batch_host: device -> host copies of the chunk on the copy stream
+struct HostSink {
+    float *sum;
+    uint32_t *count;
+    float *norm;
+    int64_t nperiods;
+    cudaError_t err;
+};
+
+int host_sink_chunk(const gpfc_chunk *ch, void *stream, void *user)
+{
+    HostSink *hs = static_cast<HostSink *>(user);
+    cudaStream_t cs = static_cast<cudaStream_t>(stream);
+    const size_t off = ((size_t)ch->curve0 * (size_t)hs->nperiods + (size_t)ch->period0) * (size_t)ch->nbins;
+    const size_t bytes = (size_t)ch->ncurves * (size_t)ch->nperiods * (size_t)ch->nbins * 4;
+    cudaError_t e = cudaSuccess;
+    if (hs->sum) e = cudaMemcpyAsync(hs->sum + off, ch->sum, bytes, cudaMemcpyDeviceToHost, cs);
+    if (e == cudaSuccess && hs->count)
+        e = cudaMemcpyAsync(hs->count + off, ch->count, bytes, cudaMemcpyDeviceToHost, cs);
+    if (e == cudaSuccess && hs->norm)
+        e = cudaMemcpyAsync(hs->norm + off, ch->norm, bytes, cudaMemcpyDeviceToHost, cs);
+    hs->err = e;
+    return e == cudaSuccess ? 0 : 1;
+}
+
+}  // namespace
+
 int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *offsets,
                          int64_t ncurves, int64_t n_total, const double *periods,
                          int64_t nperiods, int nbins, const double *t0, float *out_sum,
                          uint32_t *out_count, float *out_norm)
 {
-    // Streaming host path: inputs go up once; the curves are folded in chunks whose outputs
-    // land in one of two device slabs, and the device->host copy of chunk k (copy stream)
-    // overlaps the fold of chunk k+1 (the caller's stream).
+    // Streaming host path: inputs go up once; gpfc_fold_stream folds the batch in chunks whose
+    // outputs land in one of two device slabs, and the device->host copy of chunk k (copy
+    // stream) overlaps the fold of chunk k+1 (the caller's stream).
     if (ncurves < 0 || nperiods < 0 || n_total < 0)
         return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
     if (nbins < 1 || nbins > GPFC_MAX_NBINS)
@@ -507,20 +666,15 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
     for (int64_t c = 0; c < ncurves; ++c)
         if (offsets[c + 1] < offsets[c] || offsets[c] < 0 || offsets[c + 1] > n_total)
             return fail(GPFC_ERR_INVALID_ARG, "offsets must be non-decreasing within [0, n_total]%s");
+    const int outputs = (out_sum ? GPFC_OUT_SUM : 0) | (out_count ? GPFC_OUT_COUNT : 0) |
+                        (out_norm ? GPFC_OUT_NORM : 0);
+    if (!outputs) return GPFC_OK;
     cudaStream_t st = g_ts.stream;
-    const int nout = (out_sum ? 1 : 0) + (out_count ? 1 : 0) + (out_norm ? 1 : 0);
-    const size_t row = (size_t)nperiods * (size_t)nbins;      // elements per curve and array
-    // chunk: about 512 MB of output per slab, at least one curve
-    int64_t chunk = nout ? (int64_t)((size_t)(512u << 20) / (row * 4 * (size_t)nout)) : ncurves;
-    if (chunk < 1) chunk = 1;
-    if (chunk > ncurves) chunk = ncurves;
     const size_t b_t = align_up((size_t)n_total * 8), b_f = align_up((size_t)n_total * 4);
     const size_t b_o = align_up((size_t)(ncurves + 1) * 8), b_p = align_up((size_t)nperiods * 8);
     const size_t b_t0 = t0 ? align_up((size_t)ncurves * 8) : 0;
-    const size_t b_arr = align_up((size_t)chunk * row * 4);
-    const size_t total = b_t + b_f + b_o + b_p + b_t0 + 2 * (size_t)nout * b_arr + 256;
     char *base = nullptr;
-    cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&base), total, st);
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&base), b_t + b_f + b_o + b_p + b_t0 + 256, st);
     if (e != cudaSuccess) {
         cuda_fail(e, "device buffer allocation");
         return GPFC_ERR_WORKSPACE;
@@ -532,21 +686,8 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
     double *d_p = reinterpret_cast<double *>(cur); cur += b_p;
     double *d_t0 = nullptr;
     if (t0) { d_t0 = reinterpret_cast<double *>(cur); cur += b_t0; }
-    char *slab[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
-    for (int s = 0; s < 2; ++s)
-        for (int k = 0; k < 3; ++k) {
-            const bool want = (k == 0 && out_sum) || (k == 1 && out_count) || (k == 2 && out_norm);
-            if (want) { slab[s][k] = cur; cur += b_arr; }
-        }
-
     cudaStream_t cs = nullptr;
-    cudaEvent_t done[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr};
     e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
-    for (int s = 0; s < 2 && e == cudaSuccess; ++s) {
-        e = cudaEventCreateWithFlags(&done[s], cudaEventDisableTiming);
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&freed[s], cudaEventDisableTiming);
-    }
-    int rc = GPFC_OK;
     if (e == cudaSuccess && n_total > 0) {
         e = cudaMemcpyAsync(d_t, times, (size_t)n_total * 8, cudaMemcpyHostToDevice, st);
         if (e == cudaSuccess)
@@ -558,41 +699,17 @@ int gpfc_fold_batch_host(const double *times, const float *flux, const int64_t *
         e = cudaMemcpyAsync(d_p, periods, (size_t)nperiods * 8, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess && t0)
         e = cudaMemcpyAsync(d_t0, t0, (size_t)ncurves * 8, cudaMemcpyHostToDevice, st);
-    int64_t k = 0;
-    for (int64_t c0 = 0; c0 < ncurves && e == cudaSuccess && rc == GPFC_OK; c0 += chunk, ++k) {
-        const int s = (int)(k & 1);
-        const int64_t nc = (ncurves - c0 < chunk) ? ncurves - c0 : chunk;
-        if (k >= 2) e = cudaStreamWaitEvent(st, freed[s], 0);     // slab s copied out
-        if (e != cudaSuccess) break;
-        // the prepass scratch covers the samples offsets[c0] .. offsets[c0 + nc]: pass the
-        // whole arrays (offsets are absolute) and size the scratch by n_total
-        FoldOut o;
-        o.sum = reinterpret_cast<float *>(slab[s][0]);
-        o.count = reinterpret_cast<uint32_t *>(slab[s][1]);
-        o.norm = reinterpret_cast<float *>(slab[s][2]);
-        rc = fold_device(d_t, d_f, d_o + c0, nc, n_total, d_p, nperiods, nbins,
-                         d_t0 ? d_t0 + c0 : nullptr, 0.0, o);
-        if (rc != GPFC_OK) break;
-        e = cudaEventRecord(done[s], st);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, done[s], 0);
-        const size_t bytes = (size_t)nc * row * 4, off = (size_t)c0 * row;
-        if (e == cudaSuccess && out_sum)
-            e = cudaMemcpyAsync(out_sum + off, slab[s][0], bytes, cudaMemcpyDeviceToHost, cs);
-        if (e == cudaSuccess && out_count)
-            e = cudaMemcpyAsync(out_count + off, slab[s][1], bytes, cudaMemcpyDeviceToHost, cs);
-        if (e == cudaSuccess && out_norm)
-            e = cudaMemcpyAsync(out_norm + off, slab[s][2], bytes, cudaMemcpyDeviceToHost, cs);
-        if (e == cudaSuccess) e = cudaEventRecord(freed[s], cs);
-    }
+    int rc = GPFC_OK;
+    HostSink hs{out_sum, out_count, out_norm, nperiods, cudaSuccess};
+    if (e == cudaSuccess)
+        rc = gpfc_fold_stream(d_t, d_f, d_o, ncurves, n_total, d_p, nperiods, nbins, d_t0, outputs, 0, cs,
+                              host_sink_chunk, &hs);
     cudaError_t e2 = cs ? cudaStreamSynchronize(cs) : cudaSuccess;
     cudaError_t e3 = cudaStreamSynchronize(st);
     cudaFreeAsync(base, st);
-    for (int s = 0; s < 2; ++s) {
-        if (done[s]) cudaEventDestroy(done[s]);
-        if (freed[s]) cudaEventDestroy(freed[s]);
-    }
     if (cs) cudaStreamDestroy(cs);
-    if (rc != GPFC_OK) return rc;
+    if (e == cudaSuccess && hs.err != cudaSuccess) e = hs.err;
+    if (e == cudaSuccess && rc != GPFC_OK) return rc;
     if (e == cudaSuccess) e = e2;
     if (e == cudaSuccess) e = e3;
     if (e != cudaSuccess) return cuda_fail(e, "host-buffer fold");

@@ -41,13 +41,19 @@ def check_merge(gp, ref, s32, cnt, nb2):
                            want64=True)[1]
     err = np.abs(norm.reshape(-1, nb2) - on)
     tol = 1e-4 * np.maximum(1.0, np.abs(on))
-    # every row is compared, except a profile whose spread is below 1e-9 of its magnitude: that
-    # spread is the rounding noise of two fp64 evaluation orders of equal means (the scale of
-    # such a profile is undefined; exactly flat profiles give mu on both sides and ARE compared)
+    # Every row is compared, except profiles whose spread is at the rounding level of their
+    # own means.  Bound: either side's merged means carry a relative rounding error of a few
+    # ulp (<= 4 eps each, eps = 2^-53), so two correct evaluations differ by delta <= 8 eps mag,
+    # and (m - mu)/s turns that into 8 eps mag / s: above the 1e-4 tolerance only when
+    # s < 8 eps mag / 1e-4 ~ 1e-11 mag.  Such rows (none in the folded-curve tests, asserted
+    # there; here: equal means whose spread is one rounding) have no defined scale -- dividing
+    # rounding noise by its own std gives O(1) numbers on either side -- so only finiteness
+    # is required of them.
     sd = omean.reshape(-1, nb2).std(axis=-1)
     mag = np.abs(omean.reshape(-1, nb2)).max(axis=-1)
-    ok_rows = (sd > 1e-9 * mag) | (sd == 0)
+    ok_rows = (sd >= 1e-11 * mag) | (sd == 0)
     assert np.all(err[ok_rows] <= tol[ok_rows]), float((err[ok_rows] / tol[ok_rows]).max())
+    assert np.all(np.isfinite(norm))
     return mean, omean, int(ok_rows.sum())
 
 
@@ -126,9 +132,11 @@ def check_fused(gp, ref, times, flux, periods, nb1, nb2, t0=None, offsets=None, 
             assert np.all(np.abs(mean[c] - omean) <= 2e-7 * scale + 1e-12)
         tol = 1e-4 * np.maximum(1.0, np.abs(onorm))
         err = np.abs(norm[c] - onorm)
-        # a profile whose spread is pure rounding noise of equal means has no defined scale
+        # a profile whose spread is the rounding noise of equal means has no defined scale
+        # (bound as in check_merge: below 1e-11 of the magnitude the 1e-4 bar cannot hold for
+        # two correct evaluation orders; happens when every point sits in one intermediary bin)
         sd = omean.std(axis=-1)
-        defined = sd > 1e-9 * np.abs(omean).max(axis=-1)
+        defined = sd >= 1e-11 * np.abs(omean).max(axis=-1)
         assert np.all(err[defined] <= tol[defined]), float((err[defined] / tol[defined]).max())
         assert np.all(norm[c][~has] == 0) and np.all(mean[c][~has] == 0)
     return mean, norm
