@@ -65,6 +65,11 @@ static_assert(PK_WARPS * PK_GRAN * 8 <= PK_SCR_BYTES, "staging scratch");
 static_assert(PK_SMEM_BYTES <= 227 * 1024, "shared memory budget");
 static_assert(GPFC_TILE == 2 * PK_GRAN, "half-tile work units are one staging granule");
 
+template <bool B>
+struct PkBool {
+    static constexpr bool value = B;
+};
+
 template <int ROWLOG>
 struct PkV {
     static constexpr int ROWS = 1 << ROWLOG, HALF = ROWS / 2;
@@ -385,7 +390,13 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
         const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
         const bool ok = live && valid;
 
-        if (a.nb2 == 0) {
+        // The epilogues are compiled twice / four times: with and without the 32-bit side
+        // counts (only ever present after a count-overflow refold), and for nbins == ROWS
+        // (one row per bin) separately, so that the common case carries no dead branches.
+        auto bins_epilogue = [&](auto side_c, auto m1_c) {
+            constexpr bool SIDE = decltype(side_c)::value;
+            constexpr bool M1 = decltype(m1_c)::value;
+            const int MM = M1 ? 1 : M;
             // ---- epilogue (1): bins.  Lane (slot, p) takes the bins blk * 8 SL + e * SL + slot,
             // e = 0..7, of period p: rows of different slots differ mod SL (conflict-free).
             double *ps1 = reinterpret_cast<double *>(smem + PK_PS1_OFF);
@@ -407,10 +418,10 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                     const int bin = blk * 8 * SL + e * SL + slot;
                     int S = 0;
                     unsigned c = 0;
-                    for (int jj = 0; jj < M; ++jj) {
-                        const int row = bin * M + jj;
+                    for (int jj = 0; jj < MM; ++jj) {
+                        const int row = bin * MM + jj;
                         S += (int)H[row * PL + p];
-                        c += pk_count<ROWLOG>(H, sd, row, p);
+                        c += pk_count<ROWLOG>(H, SIDE ? sd : nullptr, row, p);
                         H[row * PL + p] = 0u;
                     }
                     if (e == 0 && bin == 0) {       // the samples at u == 0 (CurveMeta::n_zero)
@@ -435,7 +446,7 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                             kk += 1;
                             df = (float)d;
                         }
-                        H[bin * M * PL + p] = __float_as_uint(df);
+                        H[bin * MM * PL + p] = __float_as_uint(df);
                     }
                 }
                 if (live) {
@@ -496,7 +507,7 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                     float fn[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
-                        const int i0 = (blk * 8 * SL + e * SL + slot) * M * PL + p;
+                        const int i0 = (blk * 8 * SL + e * SL + slot) * MM * PL + p;
                         const float df = __uint_as_float(H[i0]);
                         H[i0] = 0u;
                         double o = base_o;
@@ -520,7 +531,9 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
             // every row has been read: clear the packed counts
             __syncthreads();
             for (int i = tid; i < HALF * PL; i += PK_THREADS) H[PK_CNT_OFF / 4 + i] = 0u;
-        } else {
+        };
+        auto merge_epilogue = [&](auto side_c) {
+            constexpr bool SIDE = decltype(side_c)::value;
             // ---- epilogue (2): equal-count merge of the nb = ROWS intermediary bins into nb2
             // bins ("Fourthly", reading R18), per period p:
             //   N = total count, per = N / nb2, target_b = per (b + 1) (= N for the last bin);
@@ -570,7 +583,7 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
 #pragma unroll
                     for (int i = 0; i < MCR; ++i) {
                         const int row = (m_lo + k) * MCR + ((i + slot) & (MCR - 1));
-                        c1 += pk_count<ROWLOG>(H, sd, row, p);
+                        c1 += pk_count<ROWLOG>(H, SIDE ? sd : nullptr, row, p);
                         q1 += (int)H[row * PL + p];
                     }
                 }
@@ -635,7 +648,7 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                     int qbef = eq[m * PL + p], q = 0;
                     int row = m * MCR;
                     for (int i = 0; i < MCR; ++i, ++row) {
-                        cnt = pk_count<ROWLOG>(H, sd, row, p);
+                        cnt = pk_count<ROWLOG>(H, SIDE ? sd : nullptr, row, p);
                         q = (int)H[row * PL + p];
                         if (cbef + cnt >= thr || i == MCR - 1) break;
                         cbef += cnt;
@@ -710,6 +723,21 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
             // clear the whole histogram
             uint4 *H4 = reinterpret_cast<uint4 *>(H);
             for (int i = tid; i < PK_HIST_BYTES / 16; i += PK_THREADS) H4[i] = make_uint4(0u, 0u, 0u, 0u);
+        };
+        using TrueT = PkBool<true>;
+        using FalseT = PkBool<false>;
+        if (a.nb2 == 0) {
+            if (sd)
+                bins_epilogue(TrueT{}, FalseT{});
+            else if (M == 1)
+                bins_epilogue(FalseT{}, TrueT{});
+            else
+                bins_epilogue(FalseT{}, FalseT{});
+        } else {
+            if (sd)
+                merge_epilogue(TrueT{});
+            else
+                merge_epilogue(FalseT{});
         }
         if (tid == 0) *ctr = 0;
         __syncthreads();   // H is zero again, tile counter reset
