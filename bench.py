@@ -61,6 +61,12 @@ def parse():
                     help="draw the light curves on the device with gpfc_make_light_curves (PAPER.md 2.6 "
                          "simulator, same shape and cadence as the config) instead of the numpy recipe; "
                          "the graded inputs are the numpy ones")
+    ap.add_argument("--nb2", type=int, default=256,
+                    help="config 5: final equal-count bins (256 = the paper's; a value the fused kernel "
+                         "does not cover, e.g. 300, runs fold + merge_equal_count_kernel: profiling)")
+    ap.add_argument("--standalone-normalize", action="store_true",
+                    help="profiling: fold writes sums and counts, gpfc_normalize makes the normalised "
+                         "profiles in a second kernel (the default step fuses it into the fold)")
     ap.add_argument("--no-others", action="store_true",
                     help="skip the other_configs block of the default run (configs 1, 3, 4, 5)")
     return ap.parse_args()
@@ -276,8 +282,9 @@ def fold_kernel_name(w):
 class DeviceRun:
     """One workload resident in HBM: buffers, the step, its timing (CUDA events, max over ranks)."""
 
-    def __init__(self, gp, torch, w, generated=False, seed=0):
+    def __init__(self, gp, torch, w, generated=False, seed=0, nb2=256, standalone_normalize=False):
         self.gp, self.torch, self.w = gp, torch, w
+        self.nb2, self.standalone_normalize = nb2, standalone_normalize
         dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
         self.generator = None
         if generated:
@@ -300,7 +307,7 @@ class DeviceRun:
         else:
             self.times, self.flux, self.offsets = dev(w.times), dev(w.flux), dev(w.offsets)
         self.two_tier = (w.config_id == 5)
-        self.shape = (w.ncurves, w.nperiods, 256 if self.two_tier else w.nbins)
+        self.shape = (w.ncurves, w.nperiods, self.nb2 if self.two_tier else w.nbins)
         self.periods = torch.empty(w.nperiods, dtype=torch.float64, device="cuda")
         f32 = lambda: torch.empty(self.shape, dtype=torch.float32, device="cuda")
         self.out_sum = self.out_count = self.out_norm = self.out_mean = None
@@ -320,8 +327,12 @@ class DeviceRun:
         gp, w = self.gp, self.w
         gp.gpfc_make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode, out=self.periods)
         if self.two_tier:
-            gp.gpfc_fold_two_tier(self.times, self.flux, self.offsets, self.periods, w.nbins, 256,
+            gp.gpfc_fold_two_tier(self.times, self.flux, self.offsets, self.periods, w.nbins, self.nb2,
                                   out_mean=self.out_mean, out_norm=self.out_norm)
+        elif self.standalone_normalize and self.out_sum is not None:
+            gp.gpfc_fold_batch(self.times, self.flux, self.offsets, self.periods, w.nbins,
+                               out_sum=self.out_sum, out_count=self.out_count, want=("sum", "count"))
+            gp.gpfc_normalize(self.out_sum, self.out_count, out_norm=self.out_norm)
         else:
             gp.gpfc_fold_batch(self.times, self.flux, self.offsets, self.periods, w.nbins,
                                out_sum=self.out_sum, out_count=self.out_count, out_norm=self.out_norm)
@@ -480,7 +491,8 @@ def gpu_arm(args):
 
     # ---- the headline workload
     w = make_workload(args, rank)
-    run = DeviceRun(gp, torch, w, generated=args.generated_inputs, seed=1000 + rank)
+    run = DeviceRun(gp, torch, w, generated=args.generated_inputs, seed=1000 + rank, nb2=args.nb2,
+                    standalone_normalize=args.standalone_normalize)
     generator = run.generator
     ms, prof, paths, clocks = run.timed(args.steps, args.warmup, barrier, world,
                                         ClockSampler(local) if rank == 0 else None)

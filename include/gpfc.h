@@ -293,7 +293,9 @@ int gpfc_make_light_curves(uint64_t seed, int64_t ncurves, int64_t n, const gpfc
  *                    device pointers [ncurves][nperiods][nbins] into the slab (NULL for arrays
  *                    not requested), valid for work enqueued on consumer_stream inside the
  *                    callback: the slab is folded into again once that work has run.  A
- *                    non-zero return stops the loop: GPFC_ERR_ABORTED.
+ *                    non-zero return stops the loop: GPFC_ERR_ABORTED.  The callback must not
+ *                    call the fold entry points of this library (the call in progress owns the
+ *                    thread's stream and scratch).
  * The library allocates the two slabs stream-ordered on the fold stream and frees them after
  * the consumer stream's last chunk; the host never waits.  Returns when everything is
  * enqueued.

@@ -101,6 +101,7 @@ size_t scratch_bytes(int64_t ncurves, int64_t n_total, int64_t nperiods, size_t 
     b += align_up((size_t)ncurves * sizeof(gpfc::CurveMeta));
     b += align_up((size_t)nperiods * sizeof(double));
     b += align_up(2 * sizeof(int64_t));   // offsets of the single-curve call
+    b += align_up(gpfc::PREP_PART_BYTES);
     b += align_up(side);
     return b + 256;
 }
@@ -179,6 +180,8 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
     cur += align_up((size_t)nperiods * sizeof(double));
     int64_t *own_off = reinterpret_cast<int64_t *>(cur);
     cur += align_up(2 * sizeof(int64_t));
+    s.part = reinterpret_cast<double *>(cur);
+    cur += align_up(gpfc::PREP_PART_BYTES);
     unsigned *side_p = side ? reinterpret_cast<unsigned *>(cur) : nullptr;
 
     if (!offsets) {   // single-curve entry point
@@ -187,7 +190,7 @@ int fold_device(const double *times, const float *flux, const int64_t *offsets, 
         offsets = own_off;
     }
     e = gpfc::launch_prep(times, flux, offsets, ncurves, t0v, t0_scalar, periods, nperiods,
-                          gpfc::fold_rows(nbins), s, st);
+                          gpfc::fold_rows(nbins), s, n_total, di->num_sms, st);
     if (e == cudaSuccess) {
         gpfc::FoldArgs a;
         a.u = s.u;

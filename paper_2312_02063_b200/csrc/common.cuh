@@ -15,6 +15,11 @@ namespace gpfc {
 // {iv = rint((u - a) * 2^S) (uint32), q (int32)}: |iv * 2^-S - (u - a)| <= 2^-(S+1).
 constexpr int GPFC_TILE = 128;
 
+// split prepass (prep.cu): at most PREP_NC_MAX CTAs per curve, used when ncurves * 2 <= SMs
+constexpr int PREP_NC_MAX = 32;
+constexpr int PREP_PART_DOUBLES = 16;
+constexpr size_t PREP_PART_BYTES = (size_t)160 * PREP_PART_DOUBLES * sizeof(double);   // <= 160 CTAs in all
+
 struct TileInfo {
     double a;          // min of u over the tile
     double inv_scale;  // 2^-S
@@ -48,6 +53,7 @@ struct Scratch {
     int2 *rec;         // [n_total + ncurves + 2]  {iv, q} (see GPFC_TILE)
     TileInfo *tiles;   // [n_total / GPFC_TILE + ncurves + 1]
     CurveMeta *meta;   // [ncurves]
+    double *part;      // [PREP_PART_BYTES / 8] partial results of the split prepass (prep.cu), or NULL
     double *rp;        // [nperiods] RN(1/P) * rows, NaN for a period that is not finite-positive;
                        // rows = fold_rows(nbins): 256 for nbins in {32..256}, 1024 for {512, 1024},
                        // else nbins
@@ -188,7 +194,7 @@ __device__ __forceinline__ void emit_profile(unsigned long long *slots, int nbin
 cudaError_t launch_prep(const double *times, const float *flux, const int64_t *offsets,
                         long long ncurves, const double *t0, double t0_scalar,
                         const double *periods, long long nperiods, int rows, Scratch s,
-                        cudaStream_t st);
+                        long long n_total, int sms, cudaStream_t st);
 int fold_rows(int nbins);         // fold.cu: resolution the fold kernel for `nbins` works at
 cudaError_t launch_fold(const FoldArgs &a, cudaStream_t st);
 cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st, int sms);   // fold_lp.cu: nbins 32..256
