@@ -449,3 +449,43 @@ def test_second_device_if_present(gp, ref):
             torch.cuda.synchronize(d)
             assert np.array_equal(c.cpu().numpy().view(np.uint32), r["count"])
             assert np.array_equal(s.cpu().numpy(), r["sum"])
+
+
+def test_two_host_threads_on_their_own_streams(gp, ref):
+    """The stream, the workspace, the error text and the launch counters are per calling
+    thread (gpfc.h): two threads fold different batches at the same time on their own streams
+    and each gets what a lone call gives."""
+    import threading
+    ws = [workloads.config2(ncurves=3, nperiods=400), workloads.config4(ncurves=5, nperiods=300)]
+    pers = [ref.make_period_grid(w.pmin, w.pmax, w.nperiods, w.grid_mode) for w in ws]
+    alone = [gp.gpfc_fold_batch(dev(w.times), dev(w.flux), dev(w.offsets), dev(p), w.nbins)
+             for w, p in zip(ws, pers)]
+    torch.cuda.synchronize()
+    got, errs = [None, None], []
+
+    def work(k):
+        try:
+            st = torch.cuda.Stream()
+            w, p = ws[k], pers[k]
+            with torch.cuda.stream(st):
+                t, f, o, pd = dev(w.times), dev(w.flux), dev(w.offsets), dev(p)
+                buf = torch.empty(gp.gpfc_workspace_bytes(w.ncurves, w.n_total, w.nperiods, w.nbins),
+                                  dtype=torch.uint8, device="cuda")
+                gp.gpfc_set_workspace(buf)
+                for _ in range(5):
+                    out = gp.gpfc_fold_batch(t, f, o, pd, w.nbins)
+                gp.gpfc_set_workspace(None)
+                st.synchronize()
+            got[k] = out
+        except BaseException as exc:      # surfaced in the main thread
+            errs.append(exc)
+
+    th = [threading.Thread(target=work, args=(k,)) for k in range(2)]
+    for t_ in th:
+        t_.start()
+    for t_ in th:
+        t_.join()
+    assert not errs, errs
+    for k in range(2):
+        for x, y in zip(got[k], alone[k]):
+            assert torch.equal(x, y)
