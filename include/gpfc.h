@@ -36,8 +36,10 @@
  *   - Return value: a gpfc_status (0 = success).  On failure
  *     gpfc_last_error() describes it; outputs are then unspecified.
  *   - Sizes of 0 (n, nperiods, ncurves, nprofiles) are valid no-ops.
- *   - nbins: 1 <= nbins <= GPFC_MAX_NBINS.  Any value is accepted; powers of
- *     two take the fast path.
+ *   - nbins: 1 <= nbins <= GPFC_MAX_NBINS.  Any value is accepted; every
+ *     nbins <= 256 and the powers of two up to 4096 take the fast kernels, other
+ *     values a plain one (true division per point-period, ~100x slower, counted
+ *     by gpfc_path_counters).
  *   - Outputs are fully overwritten, layout row-major [curve][period][bin].
  *   - Data conventions (cannot be checked on the host): a sample whose time
  *     or flux is not finite is skipped (not counted); a period that is not
@@ -347,8 +349,8 @@ int gpfc_profile_read(double *fold_kernel_ms, int64_t *fold_launches, int64_t *k
 
 /*
  * Which slow paths ran since the last gpfc_profile() call (out: host int64[8]):
- *   [0] fold calls of this thread that used the generic kernel (nbins not a power of two
- *       in 32 ... 4096: one CTA per (curve, period), true division for every point-period)
+ *   [0] fold calls of this thread that used the generic kernel (nbins above 256 that is
+ *       not a power of two: one CTA per (curve, period), true division for every point-period)
  *   [1] work items (curve x group of periods) of this DEVICE that took the exact division for
  *       every point-period: unsorted times, tiles spanning huge gaps, periods far below the
  *       sampling interval

@@ -19,7 +19,7 @@ struct ThreadState {
     // gpfc_profile: CUDA-event pairs around every fold-kernel launch + launch counters
     bool profiling = false;
     long long launches = 0;           // kernels of this library launched by this thread
-    long long generic_launches = 0;   // ... of which fold_generic_kernel (nbins not a power of two >= 32)
+    long long generic_launches = 0;   // ... of which fold_generic_kernel (nbins > 256, not a power of two)
     long long unfused_two_tier = 0;   // gpfc_fold_two_tier calls that took fold + merge kernels
     std::vector<cudaEvent_t> ev;      // start, stop, start, stop, ...
 };

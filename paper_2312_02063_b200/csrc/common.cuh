@@ -201,6 +201,7 @@ cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st, int sms);   // fo
 cudaError_t launch_fold_pk(const FoldArgs &a, cudaStream_t st, int sms);   // fold_pk.cu: nbins 512..4096
 cudaError_t launch_fold_generic(const FoldArgs &a, cudaStream_t st, int sms);   // fold.cu: any nbins
 bool fold_lp_handles(int nbins);
+bool fold_lp_pow2(int nbins);
 bool fold_pk_handles(int nbins);
 int fold_pk_rows(int nbins);
 bool fold_pk_can_merge(int nbins, int nb2);      // the fused equal-count merge fits in shared memory

@@ -1,7 +1,7 @@
 // Dispatch of the fold (PAPER.md:111 steps 1-3 and 5; noise normalisation :63 fused into the
-// epilogues) and the generic kernel.  The tuned kernels live in fold_lp.cu (nbins 32 ... 256,
-// lane = period) and fold_pk.cu (nbins 512 ... 4096, packed counts, optional fused equal-count
-// merge); every other nbins in [1, 4096] takes fold_generic_kernel below: one CTA per
+// epilogues) and the generic kernel.  The tuned kernels live in fold_lp.cu (any nbins up to 256,
+// lane = period) and fold_pk.cu (nbins 512 ... 4096, powers of two, packed counts, optional
+// fused equal-count merge); every other nbins in [257, 4096] takes fold_generic_kernel below: one CTA per
 // (curve, period), the exact formula (true division) for every point-period.  It is the
 // correctness path for bin counts that are not a power of two, not a tuned one; launches of
 // it are counted (gpfc_profile_read) so that a caller can see when it was taken.
@@ -63,7 +63,7 @@ fold_generic_kernel(FoldArgs a, long long nitems)
 
 int fold_rows(int nbins)
 {
-    if (fold_lp_handles(nbins)) return 256;
+    if (fold_lp_handles(nbins)) return fold_lp_pow2(nbins) ? 256 : 1;
     if (fold_pk_handles(nbins)) return fold_pk_rows(nbins);
     return nbins;
 }

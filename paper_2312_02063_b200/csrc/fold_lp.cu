@@ -104,12 +104,19 @@ __device__ __forceinline__ double div_by_count(double sq, unsigned c)
 // (one more integer add per point-period, same results), so nothing depends on it.
 constexpr unsigned LP_WINDOW_BASE = 0x400;
 
-template <int r, bool IMM>
+template <int r, bool IMM, bool GEN>
 __device__ __forceinline__ void pp_update(double v, int q, double rp, double C, unsigned lane4,
-                                          unsigned sbase, unsigned &gmin)
+                                          unsigned sbase, unsigned &gmin, unsigned nbu)
 {
     double m = __fma_rd(v, rp, C);
     unsigned lo = (unsigned)__double2loint(m), hi = (unsigned)__double2hiint(m);
+    if constexpr (GEN) {
+        // any nbins <= 256: m counts cycles, lo = frac(u / P) 2^32; bin = floor(phi nbins) is
+        // the high word of lo * nbins, the low word is the position inside the bin
+        const unsigned long long pr = (unsigned long long)lo * nbu;
+        lo = (unsigned)pr;
+        hi = (unsigned)(pr >> 32);
+    }
     gmin = min(gmin, lo);
     unsigned addr = __byte_perm(lane4, hi, 0x3240);      // (row << 8) | (lane << 2)
     if (IMM) {
@@ -122,20 +129,20 @@ __device__ __forceinline__ void pp_update(double v, int q, double rp, double C, 
     }
 }
 
-template <int r0, bool IMM>
+template <int r0, bool IMM, bool GEN>
 struct ForR {
     __device__ __forceinline__ static void run(double v, int q, const double (&rp)[LP_R],
                                                const double (&C)[LP_R], unsigned lane4,
-                                               unsigned sbase, unsigned (&gmin)[LP_R])
+                                               unsigned sbase, unsigned (&gmin)[LP_R], unsigned nbu)
     {
         if constexpr (r0 < LP_R) {
-            pp_update<r0, IMM>(v, q, rp[r0], C[r0], lane4, sbase, gmin[r0]);
-            ForR<r0 + 1, IMM>::run(v, q, rp, C, lane4, sbase, gmin);
+            pp_update<r0, IMM, GEN>(v, q, rp[r0], C[r0], lane4, sbase, gmin[r0], nbu);
+            ForR<r0 + 1, IMM, GEN>::run(v, q, rp, C, lane4, sbase, gmin, nbu);
         }
     }
 };
 
-template <bool IMM>
+template <bool IMM, bool GEN>
 __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroups, long long nitems,
                                              unsigned char *smem, unsigned sbase)
 {
@@ -155,10 +162,15 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
     if (tid == 0) *ctr = 0;
     __syncthreads();
 
-    const int nb = a.nbins;                      // power of two, 32 <= nb <= LP_ROWS
-    const int mshift = LP_ROWLOG - (31 - __clz(nb));   // rows merged per bin = 1 << mshift
+    // !GEN: nb a power of two, 32 <= nb <= LP_ROWS, folded at LP_ROWS rows (rp = LP_ROWS / P).
+    // GEN: any 1 <= nb <= LP_ROWS, one row per bin, the DFMA counts cycles (rp = 1 / P).
+    const int nb = a.nbins;
+    const unsigned nbu = (unsigned)nb;
+    const int mshift = GEN ? 0 : LP_ROWLOG - (31 - __clz(nb));   // rows merged per bin = 1 << mshift
     const int M = 1 << mshift;
-    const double M2 = 1729382256910270464.0;     // 1.5 * 2^(52 + ROWLOG): ulp = LP_ROWS
+    const int xrows = GEN ? nb : LP_ROWS;        // bins of the exact formula at the kernel's resolution
+    // 1.5 * 2^52 * (rows per cycle): ulp = LP_ROWS (or 1), so that w - M2 = rows floor(a rp / rows)
+    const double M2 = GEN ? 6755399441055744.0 : 1729382256910270464.0;
     const bool want_norm = a.out_norm != nullptr;
     const bool vec = a.vec_ok != 0;
 
@@ -243,40 +255,48 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
 #pragma unroll 1
                         for (int s = 0; s < LP_GRAN / 2; s += 2) {
                             const int4 ra = stage[s], rb = stage[s + 1];
-                            ForR<0, IMM>::run((double)(unsigned)ra.x, ra.y, rps, C, lane4, sbase, gmin);
-                            ForR<0, IMM>::run((double)(unsigned)ra.z, ra.w, rps, C, lane4, sbase, gmin);
-                            ForR<0, IMM>::run((double)(unsigned)rb.x, rb.y, rps, C, lane4, sbase, gmin);
-                            ForR<0, IMM>::run((double)(unsigned)rb.z, rb.w, rps, C, lane4, sbase, gmin);
+                            ForR<0, IMM, GEN>::run((double)(unsigned)ra.x, ra.y, rps, C, lane4, sbase, gmin, nbu);
+                            ForR<0, IMM, GEN>::run((double)(unsigned)ra.z, ra.w, rps, C, lane4, sbase, gmin, nbu);
+                            ForR<0, IMM, GEN>::run((double)(unsigned)rb.x, rb.y, rps, C, lane4, sbase, gmin, nbu);
+                            ForR<0, IMM, GEN>::run((double)(unsigned)rb.z, rb.w, rps, C, lane4, sbase, gmin, nbu);
                         }
                     } else {
                         const int2 *st2 = reinterpret_cast<const int2 *>(stage);
 #pragma unroll 1
                         for (int s = 0; s < gc; ++s) {
                             const int2 rc = st2[s];
-                            ForR<0, IMM>::run((double)(unsigned)rc.x, rc.y, rps, C, lane4, sbase, gmin);
+                            ForR<0, IMM, GEN>::run((double)(unsigned)rc.x, rc.y, rps, C, lane4, sbase, gmin, nbu);
                         }
                     }
                 }
                 unsigned gall = gmin[0];
 #pragma unroll
                 for (int r = 1; r < LP_R; ++r) gall = min(gall, gmin[r]);
-                if (__any_sync(0xffffffffu, gall < D)) {
+                // GEN: the guard band is D units of 2^-32 cycle = D nb units of 2^-32 bin (< 2^28)
+                const unsigned Dn = GEN ? D * nbu : D;
+                if (__any_sync(0xffffffffu, gall < Dn)) {
                     // rare: some row coordinate sat within the guard band of an integer.
                     // Re-check those samples against the exact formula; move the ones that
                     // the fast path put in the wrong row.
                     const double *us = a.u + cm.start + base;
 #pragma unroll
                     for (int r = 0; r < LP_R; ++r) {
-                        if (gmin[r] >= D || !valid[r]) continue;
+                        if (gmin[r] >= Dn || !valid[r]) continue;
                         const double per = a.periods[p0 + r * 32 + lane];
                         if (a.stats) atomicAdd(a.stats + 1, 1ull);
 #pragma unroll 4
                         for (int s = 0; s < cnt; ++s) {
                             const int2 rc = __ldg(src + s);
                             double m = __fma_rd((double)(unsigned)rc.x, rps[r], C[r]);
-                            if ((unsigned)__double2loint(m) < D) {
-                                int kf = __double2hiint(m) & (LP_ROWS - 1);
-                                int ke = exact_bin(us[s], per, LP_ROWS);
+                            unsigned flo = (unsigned)__double2loint(m);
+                            int kf = __double2hiint(m) & (LP_ROWS - 1);
+                            if constexpr (GEN) {
+                                const unsigned long long pr = (unsigned long long)flo * nbu;
+                                flo = (unsigned)pr;
+                                kf = (int)(pr >> 32);
+                            }
+                            if (flo < Dn) {
+                                int ke = exact_bin(us[s], per, xrows);
                                 if (ke != kf) {
                                     hist_update(H, r, kf, lane, rc.y, -1);
                                     if (ke >= 0) hist_update(H, r, ke, lane, rc.y, +1);
@@ -309,7 +329,7 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
 #pragma unroll
                     for (int r = 0; r < LP_R; ++r) {
                         if (valid[r]) {
-                            int ke = exact_bin(ui, per[r], LP_ROWS);
+                            int ke = exact_bin(ui, per[r], xrows);
                             if (ke >= 0) hist_update(H, r, ke, lane, qi, +1);
                         }
                     }
@@ -323,7 +343,8 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
         // slot r = g, its LP_WPR warps split the octets of bins (one 32-byte sector per output
         // array and lane).
         const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
-        const int octs = nb >> 3;
+        const int octs = (nb + 7) >> 3;               // GEN: the last octet may be partial
+        const bool vec8 = vec && !(nb & 7);
         const int r = warp / LP_WPR, wr = warp - r * LP_WPR;
         const long long j = p0 + r * 32 + lane;
         const bool live = j < a.nperiods;
@@ -381,7 +402,7 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                 }
                 if (live) {
                     const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
-                    if (vec) {
+                    if (vec8) {
                         if (a.out_sum) {
                             float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
                             o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
@@ -396,6 +417,7 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                         // outputs that are only 4-byte aligned: scalar stores
 #pragma unroll
                         for (int e = 0; e < 8; ++e) {
+                            if (GEN && oct * 8 + e >= nb) break;
                             if (a.out_sum) a.out_sum[off + e] = fs[e];
                             if (a.out_count) a.out_count[off + e] = fc[e];
                         }
@@ -448,13 +470,14 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                 }
                 if (live) {
                     float *on = a.out_norm + ((curve * a.nperiods + j) * nb) + oct * 8;
-                    if (vec) {
+                    if (vec8) {
                         float4 *o4 = reinterpret_cast<float4 *>(on);
                         o4[0] = make_float4(fn[0], fn[1], fn[2], fn[3]);
                         o4[1] = make_float4(fn[4], fn[5], fn[6], fn[7]);
                     } else {
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) on[e] = fn[e];
+                        for (int e = 0; e < 8; ++e)
+                            if (!GEN || oct * 8 + e < nb) on[e] = fn[e];
                     }
                 }
             }
@@ -464,25 +487,34 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
     }
 }
 
+template <bool GEN>
 __global__ void __launch_bounds__(LP_THREADS, 1)
 fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     const unsigned sbase = (unsigned)__cvta_generic_to_shared(smem);
     if (sbase == LP_WINDOW_BASE)
-        fold_lp_body<true>(a, ngroups, nitems, smem, sbase);
+        fold_lp_body<true, GEN>(a, ngroups, nitems, smem, sbase);
     else
-        fold_lp_body<false>(a, ngroups, nitems, smem, sbase);
+        fold_lp_body<false, GEN>(a, ngroups, nitems, smem, sbase);
 }
 
 }  // namespace
 
-bool fold_lp_handles(int nbins) { return nbins == 32 || nbins == 64 || nbins == 128 || nbins == 256; }
+bool fold_lp_handles(int nbins) { return nbins >= 1 && nbins <= LP_ROWS; }
+
+// powers of two from 32 fold at 256 rows (masks instead of a multiply); anything else up to
+// 256 bins takes the one-row-per-bin variant
+bool fold_lp_pow2(int nbins) { return nbins == 32 || nbins == 64 || nbins == 128 || nbins == 256; }
 
 cudaError_t fold_lp_init_device()
 {
-    return cudaFuncSetAttribute(fold_lp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                LP_SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(fold_lp_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         LP_SMEM_BYTES);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(fold_lp_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 LP_SMEM_BYTES);
+    return e;
 }
 
 cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st, int sms)
@@ -490,7 +522,10 @@ cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st, int sms)
     const long long ngroups = (a.nperiods + LP_GROUP - 1) / LP_GROUP;
     const long long nitems = ngroups * a.ncurves;
     const long long grid = nitems < sms ? nitems : sms;
-    fold_lp_kernel<<<(unsigned)grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems);
+    if (fold_lp_pow2(a.nbins))
+        fold_lp_kernel<false><<<(unsigned)grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems);
+    else
+        fold_lp_kernel<true><<<(unsigned)grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems);
     note_launch();
     return cudaGetLastError();
 }

@@ -120,6 +120,29 @@ def test_generic_nbins(gp, ref, nbins):
     check(g, r, exact_sums=True)
 
 
+@pytest.mark.parametrize("nbins", [1, 3, 8, 31, 33, 100, 200, 250, 255])
+def test_any_nbins_up_to_256_on_the_fast_kernel(gp, ref, nbins):
+    """nbins <= 256 that are not a power of two >= 32 run on fold_lp_kernel<true> (bin =
+    high word of frac(u/P) 2^32 * nbins), not on the generic kernel: Kepler-shaped curve with
+    many tiles and a ragged tail, 37 periods incl. cadence-commensurate ones, all outputs."""
+    w = workloads.config1(nperiods=37)
+    grid = ref.make_period_grid(w.pmin, w.pmax, 200000, w.grid_mode)
+    dt = workloads.KEPLER_CADENCE_D
+    periods = np.concatenate([grid[np.linspace(0, 199999, 30).astype(int)],
+                              [10 * dt, 12 * dt, 16 * dt, 20 * dt, 0.5, 0.25, 1.0]])
+    w.nbins = nbins
+    gp.gpfc_profile(False)
+    g = run_gpu(gp, w, periods)
+    c = gp.gpfc_path_counters()
+    assert c["generic_kernel_calls"] == 0 and c["exact_path_items"] == 0
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
+    check(g, r, exact_sums=True)
+    # fused normalisation only
+    g2 = run_gpu(gp, w, periods, want=("norm",))
+    err = np.abs(g2["norm"].astype(np.float64) - r["norm64"])
+    assert np.all(err <= 1e-4 * np.maximum(1.0, np.abs(r["norm64"])))
+
+
 @pytest.mark.parametrize("nbins", [64, 100, 256])
 def test_ragged_batch_edge_cases(gp, ref, nbins):
     """Empty and tiny curves, irregular times, negative t - t0, non-finite samples,
@@ -184,6 +207,20 @@ def test_guard_band_samples_match_division(gp, ref):
         w.nbins = nbins
         g = run_gpu(gp, w, periods)
         r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
+        check(g, r, exact_sums=True)
+    # bin counts that are not a power of two: the oracle rounds phi * nbins once, so an edge
+    # sample can land on either side of k / nbins; edges of 100, 96 and 255 bins and neighbours
+    for nbins in (100, 96, 255, 3):
+        ts = [np.zeros(2)]
+        for p in periods[:12]:
+            k = rng.integers(0, 200000, 300)
+            e = (k * p) / nbins
+            ts += [e, np.nextafter(e, np.inf), np.nextafter(e, -np.inf), k.astype(np.float64) * p]
+        t = np.sort(np.concatenate(ts))
+        f = rng.integers(-1000, 1000, t.shape[0]).astype(np.float32) * np.float32(2.0 ** -20)
+        w2 = workloads._pack("edges", -1, [(t, f, None)], 0.2, 1.0, periods.shape[0], nbins, False)
+        g = run_gpu(gp, w2, periods)
+        r = ref.fold_batch(w2.times, w2.flux, w2.offsets, periods, nbins)
         check(g, r, exact_sums=True)
 
 
@@ -367,10 +404,11 @@ def test_unsorted_and_duplicate_times(gp, ref, nbins):
         assert np.array_equal(c.cpu().numpy().view(np.uint32), rc)
         assert np.array_equal(s.cpu().numpy(), rs)       # exact integer sums: order-free
     counters = gp.gpfc_path_counters()
-    if nbins == 100:
-        assert counters["generic_kernel_calls"] == 3
-    else:
-        assert counters["exact_path_items"] > 0          # the shuffled call took the exact path
+    assert counters["generic_kernel_calls"] == 0
+    if nbins != 100:
+        # the shuffled call took the exact path (at 100 bins the DFMA counts cycles, not rows:
+        # even a tile spanning the whole baseline stays inside the fast path's range)
+        assert counters["exact_path_items"] > 0
 
 
 def test_outputs_with_4_byte_alignment(gp, ref):
