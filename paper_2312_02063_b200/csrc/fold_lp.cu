@@ -40,6 +40,10 @@ constexpr int LP_THREADS = 768, LP_WARPS = LP_THREADS / 32;
 constexpr int LP_GROUP = 32 * LP_R;           // periods per work item
 constexpr int LP_WPR = LP_WARPS / LP_R;       // epilogue: warps per period slot
 constexpr int LP_GRAN = 64;                   // samples per staging granule
+#ifndef LP_UNROLL
+#define LP_UNROLL 8
+#endif
+constexpr int LP_UNROLL_C = LP_UNROLL;        // iterations (4 samples each) unrolled in the fold loop
 
 constexpr int LP_HIST_BYTES = 196608;         // [r][row][sum|count][lane] 32-bit words
 // scratch after the histograms: sample staging during the fold, statistics partials in the
@@ -104,9 +108,11 @@ __device__ __forceinline__ double div_by_count(double sq, unsigned c)
 // (one more integer add per point-period, same results), so nothing depends on it.
 constexpr unsigned LP_WINDOW_BASE = 0x400;
 
-template <int r, bool IMM, bool GEN>
-__device__ __forceinline__ void pp_update(double v, int q, double rp, double C, unsigned lane4,
-                                          unsigned sbase, unsigned &gmin, unsigned nbu)
+// row address of one point-period: (row << 8) | (lane << 2) (+ the window base unless it is an
+// immediate); keeps the smallest fraction seen in gmin
+template <bool IMM, bool GEN>
+__device__ __forceinline__ unsigned pp_addr(double v, double rp, double C, unsigned lane4,
+                                            unsigned sbase, unsigned &gmin, unsigned nbu)
 {
     double m = __fma_rd(v, rp, C);
     unsigned lo = (unsigned)__double2loint(m), hi = (unsigned)__double2hiint(m);
@@ -119,28 +125,29 @@ __device__ __forceinline__ void pp_update(double v, int q, double rp, double C, 
     }
     gmin = min(gmin, lo);
     unsigned addr = __byte_perm(lane4, hi, 0x3240);      // (row << 8) | (lane << 2)
-    if (IMM) {
-        red_add<(int)LP_WINDOW_BASE + r * 65536>(addr, q);
-        red_inc<(int)LP_WINDOW_BASE + r * 65536 + 128>(addr);
-    } else {
-        addr += sbase;
-        red_add<r * 65536>(addr, q);
-        red_inc<r * 65536 + 128>(addr);
-    }
+    if (!IMM) addr += sbase;
+    return addr;
 }
 
-template <int r0, bool IMM, bool GEN>
-struct ForR {
-    __device__ __forceinline__ static void run(double v, int q, const double (&rp)[LP_R],
-                                               const double (&C)[LP_R], unsigned lane4,
-                                               unsigned sbase, unsigned (&gmin)[LP_R], unsigned nbu)
-    {
-        if constexpr (r0 < LP_R) {
-            pp_update<r0, IMM, GEN>(v, q, rp[r0], C[r0], lane4, sbase, gmin[r0], nbu);
-            ForR<r0 + 1, IMM, GEN>::run(v, q, rp, C, lane4, sbase, gmin, nbu);
-        }
-    }
-};
+// one sample at the lane's LP_R periods: the three sums first, then the three counts (measured:
+// the pair of atomics of one row back to back is ~1 % slower)
+template <bool IMM, bool GEN>
+__device__ __forceinline__ void sample_update(double v, int q, const double (&rp)[LP_R],
+                                              const double (&C)[LP_R], unsigned lane4,
+                                              unsigned sbase, unsigned (&gmin)[LP_R], unsigned nbu)
+{
+    static_assert(LP_R == 3, "written out for three period slots");
+    constexpr int B = IMM ? (int)LP_WINDOW_BASE : 0;
+    const unsigned a0 = pp_addr<IMM, GEN>(v, rp[0], C[0], lane4, sbase, gmin[0], nbu);
+    const unsigned a1 = pp_addr<IMM, GEN>(v, rp[1], C[1], lane4, sbase, gmin[1], nbu);
+    const unsigned a2 = pp_addr<IMM, GEN>(v, rp[2], C[2], lane4, sbase, gmin[2], nbu);
+    red_add<B>(a0, q);
+    red_add<B + 65536>(a1, q);
+    red_add<B + 131072>(a2, q);
+    red_inc<B + 128>(a0);
+    red_inc<B + 65536 + 128>(a1);
+    red_inc<B + 131072 + 128>(a2);
+}
 
 template <bool IMM, bool GEN>
 __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroups, long long nitems,
@@ -252,20 +259,20 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                     __syncwarp();
                     if (g0 + LP_GRAN + 2 * lane < cnt) nx = __ldg(src4 + (g0 + LP_GRAN) / 2 + lane);
                     if (gc == LP_GRAN) {
-#pragma unroll 1
+#pragma unroll(LP_UNROLL_C)
                         for (int s = 0; s < LP_GRAN / 2; s += 2) {
                             const int4 ra = stage[s], rb = stage[s + 1];
-                            ForR<0, IMM, GEN>::run((double)(unsigned)ra.x, ra.y, rps, C, lane4, sbase, gmin, nbu);
-                            ForR<0, IMM, GEN>::run((double)(unsigned)ra.z, ra.w, rps, C, lane4, sbase, gmin, nbu);
-                            ForR<0, IMM, GEN>::run((double)(unsigned)rb.x, rb.y, rps, C, lane4, sbase, gmin, nbu);
-                            ForR<0, IMM, GEN>::run((double)(unsigned)rb.z, rb.w, rps, C, lane4, sbase, gmin, nbu);
+                            sample_update<IMM, GEN>((double)(unsigned)ra.x, ra.y, rps, C, lane4, sbase, gmin, nbu);
+                            sample_update<IMM, GEN>((double)(unsigned)ra.z, ra.w, rps, C, lane4, sbase, gmin, nbu);
+                            sample_update<IMM, GEN>((double)(unsigned)rb.x, rb.y, rps, C, lane4, sbase, gmin, nbu);
+                            sample_update<IMM, GEN>((double)(unsigned)rb.z, rb.w, rps, C, lane4, sbase, gmin, nbu);
                         }
                     } else {
                         const int2 *st2 = reinterpret_cast<const int2 *>(stage);
 #pragma unroll 1
                         for (int s = 0; s < gc; ++s) {
                             const int2 rc = st2[s];
-                            ForR<0, IMM, GEN>::run((double)(unsigned)rc.x, rc.y, rps, C, lane4, sbase, gmin, nbu);
+                            sample_update<IMM, GEN>((double)(unsigned)rc.x, rc.y, rps, C, lane4, sbase, gmin, nbu);
                         }
                     }
                 }

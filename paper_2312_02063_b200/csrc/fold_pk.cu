@@ -43,7 +43,7 @@ constexpr int PK_CTR_OFF = PK_SCR_OFF + PK_SCR_BYTES;
 constexpr int PK_SMEM_BYTES = PK_CTR_OFF + 16;
 constexpr int PK_FLUSH_TILES = 511;               // 65,408 samples between count flushes
 #ifndef PK_UNROLL
-#define PK_UNROLL 4
+#define PK_UNROLL 8
 #endif
 constexpr int PK_UNROLL_C = PK_UNROLL;          // iterations (4 samples per lane each) unrolled in the fold loop
 // scratch, fold phase: int2 stage[PK_WARPS][PK_GRAN]                       12,288 B
