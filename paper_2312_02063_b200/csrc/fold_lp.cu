@@ -56,7 +56,9 @@ constexpr int LP_MU_OFF = LP_PKK_OFF + LP_WPR * LP_GROUP * 4;    // double [GROU
 constexpr int LP_ISD_OFF = LP_MU_OFF + LP_GROUP * 8;             // double [GROUP]
 constexpr int LP_KK_OFF = LP_ISD_OFF + LP_GROUP * 8;             // int [GROUP]
 constexpr int LP_CTR_OFF = LP_KK_OFF + LP_GROUP * 4;
-constexpr int LP_SMEM_BYTES = LP_CTR_OFF + 16;
+constexpr int LP_RT_N = 1024;                 // epilogue: RN(1 / c) for the counts c < LP_RT_N
+constexpr int LP_RT_OFF = LP_CTR_OFF + 16;    // double [LP_RT_N], written once per CTA
+constexpr int LP_SMEM_BYTES = LP_RT_OFF + LP_RT_N * 8;
 static_assert(LP_SMEM_BYTES <= 227 * 1024, "shared memory budget");
 static_assert(GPFC_TILE == 2 * LP_GRAN, "half-tile work units are one staging granule");
 static_assert(LP_WARPS * LP_GRAN * 8 <= LP_MU_OFF - LP_STAGE_OFF, "staging fits in the scratch");
@@ -100,6 +102,12 @@ __device__ __forceinline__ double div_by_count(double sq, unsigned c)
     r = __fma_rn(__fma_rn(-cd, r, 1.0), r, r);
     const double q0 = __dmul_rn(sq, r);
     return __fma_rn(__fma_rn(-q0, cd, sq), r, q0);
+}
+
+// the same for a count beyond the epilogue's reciprocal table: rare, kept out of line
+__device__ __noinline__ double div_by_count_slow(double sq, unsigned c)
+{
+    return div_by_count(sq, c);
 }
 
 // Shared-window address of dynamic shared memory on sm_100a (the first KB of the window is the
@@ -167,6 +175,8 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
     int4 *stage = reinterpret_cast<int4 *>(smem + LP_STAGE_OFF) + warp * (LP_GRAN / 2);
     for (int i = tid; i < LP_HIST_BYTES / 4; i += LP_THREADS) H[i] = 0u;
     if (tid == 0) *ctr = 0;
+    double *rt = reinterpret_cast<double *>(smem + LP_RT_OFF);
+    for (int i = tid; i < LP_RT_N; i += LP_THREADS) rt[i] = __ddiv_rn(1.0, (double)i);   // [0]: inf, never used
     __syncthreads();
 
     // !GEN: nb a power of two, 32 <= nb <= LP_ROWS, folded at LP_ROWS rows (rp = LP_ROWS / P).
@@ -343,6 +353,12 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                 }
             }
         }
+        // the samples at u == 0 (CurveMeta::n_zero) are not in the sample arrays: bin 0 of every
+        // period (atomics: other warps may still be folding)
+        if (warp < LP_R && cm.n_zero > 0) {
+            atomicAdd(&H[hidx(warp, 0, 0, lane)], (unsigned)cm.q_zero);
+            atomicAdd(&H[hidx(warp, 0, 1, lane)], (unsigned)cm.n_zero);
+        }
         __syncthreads();   // A: every update of this item is in H
 
         // ---- epilogue.  Lane l reads only its own columns: conflict-free, no cross-lane
@@ -361,9 +377,9 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
             if (rr == r) ok = live && valid[rr];
         unsigned *Hr = H + r * (LP_ROWS * 64) + lane;
         {
-            // sweep 1: sums and counts out; bin mean m (of the centred flux) back into the
-            // bin's first row as an fp64 {lo, hi} (NaN = empty); one-pass moments about the
-            // curve mean (exactly zero for a flat profile).
+            // sweep 1: sums and counts out; deviation d of the bin mean from the curve mean back
+            // into the bin's first sum word as fp32 (NaN = empty), every other word cleared;
+            // one-pass moments of d (exactly zero for a flat profile).
             double s1 = 0.0, s2 = 0.0;
             int kk = 0;
             for (int oct = wr; oct < octs; oct += LP_WPR) {
@@ -380,32 +396,36 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                         h0[jj * 64] = 0u;
                         h0[jj * 64 + 32] = 0u;
                     }
-                    if (e == 0 && oct == 0) {       // the samples at u == 0 (CurveMeta::n_zero)
-                        S += cm.q_zero;
-                        c += (unsigned)cm.n_zero;
-                    }
                     if (!ok) {
                         S = 0;
                         c = 0;
                     }
                     const double sq = __dmul_rn((double)S, inv_scale);
-                    fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
+                    const double cd = (double)c;
+                    fs[e] = (float)__dadd_rn(sq, __dmul_rn(cd, center));
                     fc[e] = c;
+                    unsigned dw = 0u;
                     if (want_norm) {
-                        double m = CUDART_NAN;
-                        if (c > 0) {
-                            m = div_by_count(sq, c);
-                            const double d = __dsub_rn(m, pivot);
-                            s1 += d;
-                            s2 += __dmul_rn(d, d);
-                            kk += 1;
+                        // mean = sq / c through the table of correctly rounded reciprocals:
+                        // q0 = sq r, one residual correction (exact whenever the quotient is
+                        // representable, like div_by_count)
+                        double m;
+                        if (c < (unsigned)LP_RT_N) {
+                            const double rc = rt[c];           // c == 0: inf, discarded below
+                            const double q0 = __dmul_rn(sq, rc);
+                            m = __fma_rn(__fma_rn(-q0, cd, sq), rc, q0);
+                        } else {
+                            m = div_by_count_slow(sq, c);
                         }
-                        h0[0] = (unsigned)__double2loint(m);
-                        h0[32] = (unsigned)__double2hiint(m);
-                    } else {
-                        h0[0] = 0u;
-                        h0[32] = 0u;
+                        const bool nz = c > 0u;
+                        const double d = nz ? __dsub_rn(m, pivot) : 0.0;
+                        s1 += d;
+                        s2 += __dmul_rn(d, d);
+                        kk += nz ? 1 : 0;
+                        dw = nz ? __float_as_uint((float)d) : 0x7fc00000u;    // NaN: empty bin
                     }
+                    h0[0] = dw;
+                    h0[32] = 0u;
                 }
                 if (live) {
                     const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
@@ -460,20 +480,22 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                 st_kk[warp * 32 + lane] = kk;
             }
             __syncthreads();
-            // sweep 2: normalised profile out, rows cleared (same split as sweep 1)
+            // sweep 2: out = base + (d - dm) / s from the fp32 deviations, in fp32 (d - dm over s
+            // is a z-score of a few units, base = mu + center: each rounding is 6e-8 relative
+            // against the 1e-4 bar of the normalised profile); rows cleared (same split as sweep 1)
             const double mu = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
-            const double base_o = (ok && st_kk[r * 32 + lane] > 0) ? __dadd_rn(mu, center) : 0.0;
+            const float dmf = (float)__dsub_rn(mu, pivot), isdf = ok ? (float)isd : 0.f;
+            const float basef = (ok && st_kk[r * 32 + lane] > 0) ? (float)__dadd_rn(mu, center) : 0.f;
             for (int oct = wr; oct < octs; oct += LP_WPR) {
                 float fn[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
                     unsigned *h0 = Hr + (oct * 8 + e) * M * 64;
-                    const double m = __hiloint2double((int)h0[32], (int)h0[0]);
+                    const float df = __uint_as_float(h0[0]);
                     h0[0] = 0u;
-                    h0[32] = 0u;
-                    double o = base_o;
-                    if (m == m && isd > 0.0) o = __dadd_rn(o, __dmul_rn(__dsub_rn(m, mu), isd));
-                    fn[e] = (float)o;
+                    // NaN (empty bin) or s == 0: the profile mean
+                    const float z = __fmaf_rn(__fsub_rn(df, dmf), isdf, basef);
+                    fn[e] = (df == df && isdf > 0.f) ? z : basef;
                 }
                 if (live) {
                     float *on = a.out_norm + ((curve * a.nperiods + j) * nb) + oct * 8;

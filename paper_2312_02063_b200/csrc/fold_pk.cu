@@ -55,6 +55,14 @@ constexpr int PK_PKK_OFF = PK_PS2_OFF + PK_WARPS * 32 * 8;
 constexpr int PK_MU_OFF = PK_PKK_OFF + PK_WARPS * 32 * 4;
 constexpr int PK_ISD_OFF = PK_MU_OFF + 32 * 8;
 constexpr int PK_KK_OFF = PK_ISD_OFF + 32 * 8;
+// scratch, paired bins epilogue (1024 rows): {1 / c, c} as doubles for the counts c < PK_RT_N,
+// written once per CTA behind the other bins-epilogue scratch (the fold's staging and the
+// statistics partials stay below it; the merge epilogue, which uses the whole scratch, never
+// runs in the same launch)
+constexpr int PK_RT_N = 256;
+constexpr int PK_RT_OFF = PK_SCR_OFF + 16384;
+static_assert(PK_KK_OFF + 32 * 4 <= PK_RT_OFF, "reciprocal table behind the bins-epilogue scratch");
+static_assert(PK_RT_OFF + PK_RT_N * 16 <= PK_SCR_OFF + PK_SCR_BYTES, "reciprocal table fits");
 // scratch, merge epilogue: cumulative count / integer flux in front of every mini-chunk
 // (32 or 16 KB), warp totals [PK_WARPS][PL] (6 KB at most); the cumulative flux at the
 // boundaries goes over the histogram: [nb2 + 1][PL] doubles, PL * nb2 <= PK_MG_MAX
@@ -174,6 +182,10 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
     int4 *stage4 = reinterpret_cast<int4 *>(smem + PK_SCR_OFF) + warp * (PK_GRAN / 2);
     for (int i = tid; i < PK_HIST_WORDS; i += PK_THREADS) H[i] = 0u;
     if (tid == 0) *ctr = 0;
+    if (ROWLOG == 10 && a.nb2 == 0 && tid < PK_RT_N) {
+        double2 *rt = reinterpret_cast<double2 *>(smem + PK_RT_OFF);
+        rt[tid] = make_double2(__ddiv_rn(1.0, (double)tid), (double)tid);   // [0] is never read
+    }
     __syncthreads();
 
     const int nb = a.nbins;                               // power of two, ROWS / 2 <= nb <= ROWS
@@ -532,6 +544,193 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
             __syncthreads();
             for (int i = tid; i < HALF * PL; i += PK_THREADS) H[PK_CNT_OFF / 4 + i] = 0u;
         };
+        // ---- epilogue (1b): bins, ROWS = nbins = 1024 (SL = 1, no side counts): config 3's
+        // case.  A thread takes the bins k and k + HALF together (they share a packed count
+        // word: one load, decoded once, cleared in place), divides by the count through a
+        // table of correctly rounded reciprocals (q0 = sq r, one residual correction: exact
+        // whenever the quotient is representable, as pk_div_by_count), and sweep 2 runs in fp32.
+        auto bins_epilogue_pair = [&]() {
+            double *ps1 = reinterpret_cast<double *>(smem + PK_PS1_OFF);
+            double *ps2 = reinterpret_cast<double *>(smem + PK_PS2_OFF);
+            int *pkk = reinterpret_cast<int *>(smem + PK_PKK_OFF);
+            double *st_mu = reinterpret_cast<double *>(smem + PK_MU_OFF);
+            double *st_isd = reinterpret_cast<double *>(smem + PK_ISD_OFF);
+            int *st_kk = reinterpret_cast<int *>(smem + PK_KK_OFF);
+            const double2 *rt = reinterpret_cast<const double2 *>(smem + PK_RT_OFF);
+            const bool want_norm = a.out_norm != nullptr;
+            constexpr int NOCT = HALF / 8;                     // octets of bins per half
+            const long long orow = (curve * a.nperiods + j) * ROWS;
+            unsigned *Hc = H + PK_CNT_OFF / 4;
+            double s1 = 0.0, s2 = 0.0;
+            int kk = 0;
+            // one bin: outputs, deviation of its mean from the curve mean (fp32, NaN = empty)
+            auto one_bin = [&](int S, unsigned c, float &fs, float &df) {
+                const double sq = __dmul_rn((double)S, inv_scale);
+                double r, cd;
+                if (c < (unsigned)PK_RT_N) {
+                    const double2 t = rt[c];
+                    r = t.x;
+                    cd = t.y;
+                } else {
+                    cd = (double)c;
+                    r = __ddiv_rn(1.0, cd);
+                }
+                fs = (float)__dadd_rn(sq, __dmul_rn(cd, center));
+                df = __int_as_float(0x7fc00000);
+                if (want_norm && c > 0) {
+                    const double q0 = __dmul_rn(sq, r);
+                    const double m = __fma_rn(__fma_rn(-q0, cd, sq), r, q0);
+                    const double d = __dsub_rn(m, pivot);
+                    s1 += d;
+                    s2 += __dmul_rn(d, d);
+                    kk += 1;
+                    df = (float)d;
+                }
+            };
+            for (int oct = warp; oct < NOCT; oct += PK_WARPS) {
+                unsigned chi[8];
+                float fs[8], dfv[8];
+                unsigned fc[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int row = oct * 8 + e;
+                    const unsigned w = Hc[row * PL + p];
+                    Hc[row * PL + p] = 0u;
+                    chi[e] = w >> 16;
+                    unsigned c = (w & 0xffffu) - chi[e];
+                    int S = (int)H[row * PL + p];
+                    if (e == 0 && oct == 0) {       // the samples at u == 0 (CurveMeta::n_zero)
+                        S += cm.q_zero;
+                        c += (unsigned)cm.n_zero;
+                    }
+                    if (!ok) {
+                        S = 0;
+                        c = 0;
+                        chi[e] = 0;
+                    }
+                    fc[e] = c;
+                    one_bin(S, c, fs[e], dfv[e]);
+                    H[row * PL + p] = __float_as_uint(dfv[e]);
+                }
+                if (live) {
+                    const long long off = orow + oct * 8;
+                    if (a.vec_ok) {
+                        if (a.out_sum) {
+                            float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
+                            o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
+                            o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
+                        }
+                        if (a.out_count) {
+                            uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
+                            o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
+                            o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
+                        }
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            if (a.out_sum) a.out_sum[off + e] = fs[e];
+                            if (a.out_count) a.out_count[off + e] = fc[e];
+                        }
+                    }
+                }
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int row = HALF + oct * 8 + e;
+                    int S = (int)H[row * PL + p];
+                    if (!ok) S = 0;
+                    one_bin(S, chi[e], fs[e], dfv[e]);
+                    H[row * PL + p] = __float_as_uint(dfv[e]);
+                }
+                if (live) {
+                    const long long off = orow + HALF + oct * 8;
+                    if (a.vec_ok) {
+                        if (a.out_sum) {
+                            float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
+                            o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
+                            o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
+                        }
+                        if (a.out_count) {
+                            uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
+                            o4[0] = make_uint4(chi[0], chi[1], chi[2], chi[3]);
+                            o4[1] = make_uint4(chi[4], chi[5], chi[6], chi[7]);
+                        }
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            if (a.out_sum) a.out_sum[off + e] = fs[e];
+                            if (a.out_count) a.out_count[off + e] = chi[e];
+                        }
+                    }
+                }
+            }
+            if (!want_norm) {
+                // nothing reads the deviations: clear the sum words (this thread's own)
+                for (int oct = warp; oct < NOCT; oct += PK_WARPS)
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        H[(oct * 8 + e) * PL + p] = 0u;
+                        H[(HALF + oct * 8 + e) * PL + p] = 0u;
+                    }
+                return;
+            }
+            ps1[warp * 32 + lane] = s1;
+            ps2[warp * 32 + lane] = s2;
+            pkk[warp * 32 + lane] = kk;
+            __syncthreads();
+            if (tid < PL) {
+                double t1 = 0.0, t2 = 0.0;
+                int tk = 0;
+                for (int w = 0; w < PK_WARPS; ++w) {           // fixed order: deterministic
+                    t1 += ps1[w * 32 + tid];
+                    t2 += ps2[w * 32 + tid];
+                    tk += pkk[w * 32 + tid];
+                }
+                double mu = 0.0, isd = 0.0;
+                if (tk > 0) {
+                    const double dm = __ddiv_rn(t1, (double)tk);
+                    mu = __dadd_rn(pivot, dm);
+                    const double var = __dsub_rn(__ddiv_rn(t2, (double)tk), __dmul_rn(dm, dm));
+                    const double sdv = (var > 0.0) ? sqrt(var) : 0.0;
+                    if (tk >= 2 && sdv > 0.0) isd = __ddiv_rn(1.0, sdv);
+                }
+                st_mu[tid] = mu;
+                st_isd[tid] = isd;
+                st_kk[tid] = tk;
+            }
+            __syncthreads();
+            // sweep 2: out = base + (d - dm) / s from the fp32 deviations, in fp32 (|d - dm| / s
+            // is a z-score of a few units, base = mu + center: each rounding is 6e-8 relative,
+            // against the 1e-4 bar of the normalised profile); every thread reads back the words
+            // it wrote in sweep 1
+            const double mu = st_mu[p], isd = st_isd[p];
+            const float dmf = (float)__dsub_rn(mu, pivot), isdf = (float)isd;
+            const float basef = (ok && st_kk[p] > 0) ? (float)__dadd_rn(mu, center) : 0.f;
+            const bool scale = ok && isd > 0.0;
+            for (int oct = warp; oct < NOCT; oct += PK_WARPS) {
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    float fn[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int i0 = (h * HALF + oct * 8 + e) * PL + p;
+                        const float df = __uint_as_float(H[i0]);
+                        H[i0] = 0u;
+                        fn[e] = (scale && df == df) ? __fmaf_rn(__fsub_rn(df, dmf), isdf, basef) : basef;
+                    }
+                    if (live) {
+                        const long long off = orow + h * HALF + oct * 8;
+                        if (a.vec_ok) {
+                            float4 *o4 = reinterpret_cast<float4 *>(a.out_norm + off);
+                            o4[0] = make_float4(fn[0], fn[1], fn[2], fn[3]);
+                            o4[1] = make_float4(fn[4], fn[5], fn[6], fn[7]);
+                        } else {
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) a.out_norm[off + e] = fn[e];
+                        }
+                    }
+                }
+            }
+        };
         auto merge_epilogue = [&](auto side_c) {
             constexpr bool SIDE = decltype(side_c)::value;
             // ---- epilogue (2): equal-count merge of the nb = ROWS intermediary bins into nb2
@@ -729,8 +928,12 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
         if (a.nb2 == 0) {
             if (sd)
                 bins_epilogue(TrueT{}, FalseT{});
-            else if (M == 1)
-                bins_epilogue(FalseT{}, TrueT{});
+            else if (M == 1) {
+                if constexpr (ROWLOG == 10)
+                    bins_epilogue_pair();
+                else
+                    bins_epilogue(FalseT{}, TrueT{});
+            }
             else
                 bins_epilogue(FalseT{}, FalseT{});
         } else {
