@@ -55,7 +55,7 @@ constexpr int PK_PKK_OFF = PK_PS2_OFF + PK_WARPS * 32 * 8;
 constexpr int PK_MU_OFF = PK_PKK_OFF + PK_WARPS * 32 * 4;
 constexpr int PK_ISD_OFF = PK_MU_OFF + 32 * 8;
 constexpr int PK_KK_OFF = PK_ISD_OFF + 32 * 8;
-// scratch, paired bins epilogue (1024 rows): {1 / c, c} as doubles for the counts c < PK_RT_N,
+// scratch, lane = bin epilogue (1024 rows): {1 / c, c} as doubles for the counts c < PK_RT_N,
 // written once per CTA behind the other bins-epilogue scratch (the fold's staging and the
 // statistics partials stay below it; the merge epilogue, which uses the whole scratch, never
 // runs in the same launch)
@@ -287,35 +287,41 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                             }
                         }
                     }
-                    if (__any_sync(0xffffffffu, gmin < D)) {
-                        // rare: a row coordinate sat within the guard band of an integer.  The
-                        // flagged lanes re-check THEIR samples (same enumeration as above)
-                        // against the exact formula and move the ones in the wrong row.
-                        if (gmin < D && valid) {
-                            const double per = a.periods[j];
-                            const double *us = a.u + cm.start + base;
-                            if (a.stats) atomicAdd(a.stats + 1, 1ull);
+                    unsigned flagged = __ballot_sync(0xffffffffu, gmin < D && valid);
+                    if (flagged) {
+                        // rare: a row coordinate sat within the guard band of an integer.  For
+                        // every flagged lane (slot, period) the WHOLE warp re-checks that lane's
+                        // samples (same enumeration as above), 32 at a time, against the exact
+                        // formula and moves the ones in the wrong row.
+                        const double *us = a.u + cm.start + base;
+                        do {
+                            const int L = __ffs(flagged) - 1;
+                            flagged &= flagged - 1;
+                            const int pL = L & (PL - 1), slotL = L >> PLOG;
+                            const double rps_l = __shfl_sync(0xffffffffu, rps, L);
+                            const double C_l = __shfl_sync(0xffffffffu, C, L);
+                            const double per = a.periods[p0 + pL];
+                            if (a.stats && lane == 0) atomicAdd(a.stats + 1, 1ull);
                             for (int g0 = 0; g0 < cnt; g0 += PK_GRAN) {
                                 const int gc = min(PK_GRAN, cnt - g0);
-                                const int ns = (gc == PK_GRAN) ? PK_GRAN / SL : (gc - slot + SL - 1) / SL;
-#pragma unroll 4
-                                for (int i = 0; i < ns; ++i) {
-                                    // i-th sample of this slot in the granule
-                                    const int s = (gc == PK_GRAN) ? (((i >> 1) * SL + slot) * 2 + (i & 1))
-                                                                  : (slot + i * SL);
+                                const int ns = (gc == PK_GRAN) ? PK_GRAN / SL : (gc - slotL + SL - 1) / SL;
+                                for (int i = lane; i < ns; i += 32) {
+                                    // i-th sample of that slot in the granule
+                                    const int s = (gc == PK_GRAN) ? (((i >> 1) * SL + slotL) * 2 + (i & 1))
+                                                                  : (slotL + i * SL);
                                     const int2 rc = __ldg(src + g0 + s);
-                                    const double m = __fma_rd((double)(unsigned)rc.x, rps, C);
+                                    const double m = __fma_rd((double)(unsigned)rc.x, rps_l, C_l);
                                     if ((unsigned)__double2loint(m) < D) {
                                         const int kf = __double2hiint(m) & (ROWS - 1);
                                         const int ke = exact_bin(us[g0 + s], per, ROWS);
                                         if (ke != kf) {
-                                            pk_hist_update<ROWLOG>(H, kf, p, rc.y, -1);
-                                            if (ke >= 0) pk_hist_update<ROWLOG>(H, ke, p, rc.y, +1);
+                                            pk_hist_update<ROWLOG>(H, kf, pL, rc.y, -1);
+                                            if (ke >= 0) pk_hist_update<ROWLOG>(H, ke, pL, rc.y, +1);
                                         }
                                     }
                                 }
                             }
-                        }
+                        } while (flagged);
                     }
                 }
             } else {
@@ -545,189 +551,162 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
             for (int i = tid; i < HALF * PL; i += PK_THREADS) H[PK_CNT_OFF / 4 + i] = 0u;
         };
         // ---- epilogue (1b): bins, ROWS = nbins = 1024 (SL = 1, no side counts): config 3's
-        // case.  A thread takes the bins k and k + HALF together (they share a packed count
-        // word: one load, decoded once, cleared in place), divides by the count through a
-        // table of correctly rounded reciprocals (q0 = sq r, one residual correction: exact
-        // whenever the quotient is representable, as pk_div_by_count), and sweep 2 runs in fp32.
-        auto bins_epilogue_pair = [&]() {
-            double *ps1 = reinterpret_cast<double *>(smem + PK_PS1_OFF);
+        // case.  With lane = period every store instruction touches 32 different 128-byte
+        // lines (16 bytes each), and at 384 KB of output per work item the store unit, one line
+        // per cycle, was the bottleneck of the epilogue (ncu: long_sb / mio stalls, 14 % of the
+        // kernel).  So the arithmetic is done with lane = bin: every row vector of 32 words
+        // (sums, packed counts) is first permuted in place, column p -> p ^ (row & 31); a warp
+        // that then walks the rows 32 t + l of ONE period p reads column p ^ l -- 32 different
+        // banks -- and every store is one full line.  Unit of work = (period, third of its 32
+        // row tiles): 96 units, 4 per warp.  Bin mean through a table of correctly rounded
+        // reciprocals (q0 = sq r, one residual correction: exact whenever the quotient is
+        // representable, as pk_div_by_count); sweep 2 in fp32.
+        auto bins_epilogue_lanebin = [&](auto all_c) {
+            constexpr bool ALL = decltype(all_c)::value;    // sums, counts and normalised profile all wanted
+            double *ps1 = reinterpret_cast<double *>(smem + PK_PS1_OFF);      // [96] per unit
             double *ps2 = reinterpret_cast<double *>(smem + PK_PS2_OFF);
             int *pkk = reinterpret_cast<int *>(smem + PK_PKK_OFF);
-            double *st_mu = reinterpret_cast<double *>(smem + PK_MU_OFF);
-            double *st_isd = reinterpret_cast<double *>(smem + PK_ISD_OFF);
-            int *st_kk = reinterpret_cast<int *>(smem + PK_KK_OFF);
+            float *st_dm = reinterpret_cast<float *>(smem + PK_MU_OFF);       // [32] per period
+            float *st_isd = st_dm + 32;
+            float *st_base = st_dm + 64;
             const double2 *rt = reinterpret_cast<const double2 *>(smem + PK_RT_OFF);
-            const bool want_norm = a.out_norm != nullptr;
-            constexpr int NOCT = HALF / 8;                     // octets of bins per half
-            const long long orow = (curve * a.nperiods + j) * ROWS;
+            const bool want_norm = ALL || a.out_norm != nullptr;
+            const bool w_sum = ALL || a.out_sum != nullptr, w_cnt = ALL || a.out_count != nullptr;
             unsigned *Hc = H + PK_CNT_OFF / 4;
-            double s1 = 0.0, s2 = 0.0;
-            int kk = 0;
-            // one bin: outputs, deviation of its mean from the curve mean (fp32, NaN = empty)
-            auto one_bin = [&](int S, unsigned c, float &fs, float &df) {
-                const double sq = __dmul_rn((double)S, inv_scale);
-                double r, cd;
-                if (c < (unsigned)PK_RT_N) {
-                    const double2 t = rt[c];
-                    r = t.x;
-                    cd = t.y;
-                } else {
-                    cd = (double)c;
-                    r = __ddiv_rn(1.0, cd);
-                }
-                fs = (float)__dadd_rn(sq, __dmul_rn(cd, center));
-                df = __int_as_float(0x7fc00000);
-                if (want_norm && c > 0) {
-                    const double q0 = __dmul_rn(sq, r);
-                    const double m = __fma_rn(__fma_rn(-q0, cd, sq), r, q0);
-                    const double d = __dsub_rn(m, pivot);
-                    s1 += d;
-                    s2 += __dmul_rn(d, d);
-                    kk += 1;
-                    df = (float)d;
-                }
-            };
-            for (int oct = warp; oct < NOCT; oct += PK_WARPS) {
-                unsigned chi[8];
-                float fs[8], dfv[8];
-                unsigned fc[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int row = oct * 8 + e;
-                    const unsigned w = Hc[row * PL + p];
-                    Hc[row * PL + p] = 0u;
-                    chi[e] = w >> 16;
-                    unsigned c = (w & 0xffffu) - chi[e];
-                    int S = (int)H[row * PL + p];
-                    if (e == 0 && oct == 0) {       // the samples at u == 0 (CurveMeta::n_zero)
-                        S += cm.q_zero;
-                        c += (unsigned)cm.n_zero;
-                    }
-                    if (!ok) {
-                        S = 0;
-                        c = 0;
-                        chi[e] = 0;
-                    }
-                    fc[e] = c;
-                    one_bin(S, c, fs[e], dfv[e]);
-                    H[row * PL + p] = __float_as_uint(dfv[e]);
-                }
-                if (live) {
-                    const long long off = orow + oct * 8;
-                    if (a.vec_ok) {
-                        if (a.out_sum) {
-                            float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
-                            o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
-                            o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
-                        }
-                        if (a.out_count) {
-                            uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
-                            o4[0] = make_uint4(fc[0], fc[1], fc[2], fc[3]);
-                            o4[1] = make_uint4(fc[4], fc[5], fc[6], fc[7]);
-                        }
-                    } else {
-#pragma unroll
-                        for (int e = 0; e < 8; ++e) {
-                            if (a.out_sum) a.out_sum[off + e] = fs[e];
-                            if (a.out_count) a.out_count[off + e] = fc[e];
-                        }
-                    }
-                }
-#pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int row = HALF + oct * 8 + e;
-                    int S = (int)H[row * PL + p];
-                    if (!ok) S = 0;
-                    one_bin(S, chi[e], fs[e], dfv[e]);
-                    H[row * PL + p] = __float_as_uint(dfv[e]);
-                }
-                if (live) {
-                    const long long off = orow + HALF + oct * 8;
-                    if (a.vec_ok) {
-                        if (a.out_sum) {
-                            float4 *o4 = reinterpret_cast<float4 *>(a.out_sum + off);
-                            o4[0] = make_float4(fs[0], fs[1], fs[2], fs[3]);
-                            o4[1] = make_float4(fs[4], fs[5], fs[6], fs[7]);
-                        }
-                        if (a.out_count) {
-                            uint4 *o4 = reinterpret_cast<uint4 *>(a.out_count + off);
-                            o4[0] = make_uint4(chi[0], chi[1], chi[2], chi[3]);
-                            o4[1] = make_uint4(chi[4], chi[5], chi[6], chi[7]);
-                        }
-                    } else {
-#pragma unroll
-                        for (int e = 0; e < 8; ++e) {
-                            if (a.out_sum) a.out_sum[off + e] = fs[e];
-                            if (a.out_count) a.out_count[off + e] = chi[e];
-                        }
-                    }
-                }
+            // the item's validity per period (lane = period here) for the lane = bin phases
+            const unsigned livemask = __ballot_sync(0xffffffffu, live);
+            const unsigned okmask = __ballot_sync(0xffffffffu, ok);
+            // the samples at u == 0 (CurveMeta::n_zero) belong to row 0: warp 0 adds them to the
+            // row vectors it permutes first below
+            if (warp == 0 && cm.n_zero > 0) {
+                H[lane] += (unsigned)cm.q_zero;
+                Hc[lane] += (unsigned)cm.n_zero;
             }
-            if (!want_norm) {
-                // nothing reads the deviations: clear the sum words (this thread's own)
-                for (int oct = warp; oct < NOCT; oct += PK_WARPS)
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        H[(oct * 8 + e) * PL + p] = 0u;
-                        H[(HALF + oct * 8 + e) * PL + p] = 0u;
-                    }
-                return;
-            }
-            ps1[warp * 32 + lane] = s1;
-            ps2[warp * 32 + lane] = s2;
-            pkk[warp * 32 + lane] = kk;
-            __syncthreads();
-            if (tid < PL) {
-                double t1 = 0.0, t2 = 0.0;
-                int tk = 0;
-                for (int w = 0; w < PK_WARPS; ++w) {           // fixed order: deterministic
-                    t1 += ps1[w * 32 + tid];
-                    t2 += ps2[w * 32 + tid];
-                    tk += pkk[w * 32 + tid];
-                }
-                double mu = 0.0, isd = 0.0;
-                if (tk > 0) {
-                    const double dm = __ddiv_rn(t1, (double)tk);
-                    mu = __dadd_rn(pivot, dm);
-                    const double var = __dsub_rn(__ddiv_rn(t2, (double)tk), __dmul_rn(dm, dm));
-                    const double sdv = (var > 0.0) ? sqrt(var) : 0.0;
-                    if (tk >= 2 && sdv > 0.0) isd = __ddiv_rn(1.0, sdv);
-                }
-                st_mu[tid] = mu;
-                st_isd[tid] = isd;
-                st_kk[tid] = tk;
+            // phase A: permute the row vectors (1024 of sums, 512 of packed counts)
+#pragma unroll 4
+            for (int v = warp; v < ROWS + HALF; v += PK_WARPS) {
+                unsigned *hv = H + v * 32;                  // the counts follow the sums
+                const unsigned xw = hv[lane];
+                hv[lane ^ (v & 31)] = xw;                   // the warp's loads complete before its store issues
             }
             __syncthreads();
-            // sweep 2: out = base + (d - dm) / s from the fp32 deviations, in fp32 (|d - dm| / s
-            // is a z-score of a few units, base = mu + center: each rounding is 6e-8 relative,
-            // against the 1e-4 bar of the normalised profile); every thread reads back the words
-            // it wrote in sweep 1
-            const double mu = st_mu[p], isd = st_isd[p];
-            const float dmf = (float)__dsub_rn(mu, pivot), isdf = (float)isd;
-            const float basef = (ok && st_kk[p] > 0) ? (float)__dadd_rn(mu, center) : 0.f;
-            const bool scale = ok && isd > 0.0;
-            for (int oct = warp; oct < NOCT; oct += PK_WARPS) {
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    float fn[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        const int i0 = (h * HALF + oct * 8 + e) * PL + p;
-                        const float df = __uint_as_float(H[i0]);
-                        H[i0] = 0u;
-                        fn[e] = (scale && df == df) ? __fmaf_rn(__fsub_rn(df, dmf), isdf, basef) : basef;
+            const long long obase = (curve * a.nperiods + p0) * ROWS;
+            constexpr int UPW = 96 / PK_WARPS;                 // units per warp
+            // sweep 1
+#pragma unroll 1
+            for (int i = 0; i < UPW; ++i) {
+                const int u = warp * UPW + i;
+                const int pp = u / 3, part = u - pp * 3;
+                const int t_lo = part * 11, t_hi = min(32, t_lo + 11);
+                const bool lv = (livemask >> pp) & 1u, okp = (okmask >> pp) & 1u;
+                // running pointers (kept opaque so that they stay in registers)
+                unsigned long long po = (unsigned long long)(obase + (long long)pp * ROWS + t_lo * 32 + lane) * 4ull;
+                asm volatile("" : "+l"(po));
+                unsigned hs = (unsigned)((t_lo * 32 + lane) * 32 + (pp ^ lane));      // word index of (row, col)
+                asm volatile("" : "+r"(hs));
+                double s1 = 0.0, s2 = 0.0;
+                int kk = 0;
+#pragma unroll 2
+                for (int t = t_lo; t < t_hi; ++t) {
+                    int S = (int)H[hs];
+                    const unsigned w = Hc[hs & (HALF * 32 - 1)];
+                    unsigned c = (t >= 16) ? (w >> 16) : ((w & 0xffffu) - (w >> 16));
+                    S = okp ? S : 0;
+                    c = okp ? c : 0u;
+                    const double sq = __dmul_rn((double)S, inv_scale);
+                    double r, cd;
+                    if (c < (unsigned)PK_RT_N) {
+                        const double2 tb = rt[c];          // c == 0: {inf, 0}, discarded below
+                        r = tb.x;
+                        cd = tb.y;
+                    } else {
+                        cd = (double)c;
+                        r = __ddiv_rn(1.0, cd);
                     }
-                    if (live) {
-                        const long long off = orow + h * HALF + oct * 8;
-                        if (a.vec_ok) {
-                            float4 *o4 = reinterpret_cast<float4 *>(a.out_norm + off);
-                            o4[0] = make_float4(fn[0], fn[1], fn[2], fn[3]);
-                            o4[1] = make_float4(fn[4], fn[5], fn[6], fn[7]);
-                        } else {
-#pragma unroll
-                            for (int e = 0; e < 8; ++e) a.out_norm[off + e] = fn[e];
-                        }
+                    if (w_sum && lv)
+                        *reinterpret_cast<float *>((char *)a.out_sum + po) = (float)__dadd_rn(sq, __dmul_rn(cd, center));
+                    if (w_cnt && lv) *reinterpret_cast<uint32_t *>((char *)a.out_count + po) = c;
+                    unsigned dw = 0u;
+                    if (want_norm) {
+                        const double q0 = __dmul_rn(sq, r);
+                        const double m = __fma_rn(__fma_rn(-q0, cd, sq), r, q0);
+                        const bool nz = c > 0u;
+                        const double d = nz ? __dsub_rn(m, pivot) : 0.0;
+                        s1 += d;
+                        s2 += __dmul_rn(d, d);
+                        kk += nz ? 1 : 0;
+                        dw = nz ? __float_as_uint((float)d) : 0x7fc00000u;    // NaN: empty bin
                     }
+                    H[hs] = dw;
+                    hs += 32 * 32;
+                    po += 128;
+                }
+                if (want_norm) {
+                    s1 = warp_sum(s1);
+                    s2 = warp_sum(s2);
+                    kk = warp_sum_int(kk);
+                    if (lane == 0) {
+                        ps1[u] = s1;
+                        ps2[u] = s2;
+                        pkk[u] = kk;
+                    }
+                }
+            }
+            __syncthreads();   // every packed count word has been read (twice): they can go
+            if (want_norm) {
+                if (tid < PL) {
+                    double t1 = 0.0, t2 = 0.0;
+                    int tk = 0;
+                    for (int q3 = 0; q3 < 3; ++q3) {               // fixed order: deterministic
+                        t1 += ps1[tid * 3 + q3];
+                        t2 += ps2[tid * 3 + q3];
+                        tk += pkk[tid * 3 + q3];
+                    }
+                    double mu = 0.0, isd = 0.0;
+                    if (tk > 0) {
+                        const double dm = __ddiv_rn(t1, (double)tk);
+                        mu = __dadd_rn(pivot, dm);
+                        const double var = __dsub_rn(__ddiv_rn(t2, (double)tk), __dmul_rn(dm, dm));
+                        const double sdv = (var > 0.0) ? sqrt(var) : 0.0;
+                        if (tk >= 2 && sdv > 0.0) isd = __ddiv_rn(1.0, sdv);
+                    }
+                    // tid is the period here, as in `ok`
+                    st_dm[tid] = (float)__dsub_rn(mu, pivot);
+                    st_isd[tid] = ok ? (float)isd : 0.f;
+                    st_base[tid] = (ok && tk > 0) ? (float)__dadd_rn(mu, center) : 0.f;
+                }
+                __syncthreads();
+            }
+            // sweep 2: out = base + (d - dm) / s from the fp32 deviations, in fp32 (a z-score of a
+            // few units plus mu + center: each rounding is 6e-8 relative, the bar is 1e-4);
+            // every word of the histogram cleared
+#pragma unroll 1
+            for (int i = 0; i < UPW; ++i) {
+                const int u = warp * UPW + i;
+                const int pp = u / 3, part = u - pp * 3;
+                const int t_lo = part * 11, t_hi = min(32, t_lo + 11);
+                const bool lv = ((livemask >> pp) & 1u) && want_norm;
+                unsigned long long po = (unsigned long long)(obase + (long long)pp * ROWS + t_lo * 32 + lane) * 4ull;
+                asm volatile("" : "+l"(po));
+                unsigned hs = (unsigned)((t_lo * 32 + lane) * 32 + (pp ^ lane));
+                asm volatile("" : "+r"(hs));
+                float dmf = 0.f, isdf = 0.f, basef = 0.f;
+                if (want_norm) {
+                    dmf = st_dm[pp];
+                    isdf = st_isd[pp];
+                    basef = st_base[pp];
+                }
+#pragma unroll 2
+                for (int t = t_lo; t < t_hi; ++t) {
+                    const float df = __uint_as_float(H[hs]);
+                    H[hs] = 0u;
+                    if (t < 16) Hc[hs] = 0u;
+                    // NaN (empty bin) or s == 0: the profile mean
+                    const float z = __fmaf_rn(__fsub_rn(df, dmf), isdf, basef);
+                    const float o = (df == df && isdf > 0.f) ? z : basef;
+                    if (lv) *reinterpret_cast<float *>((char *)a.out_norm + po) = o;
+                    hs += 32 * 32;
+                    po += 128;
                 }
             }
         };
@@ -929,8 +908,12 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
             if (sd)
                 bins_epilogue(TrueT{}, FalseT{});
             else if (M == 1) {
-                if constexpr (ROWLOG == 10)
-                    bins_epilogue_pair();
+                if constexpr (ROWLOG == 10) {
+                    if (a.out_sum && a.out_count && a.out_norm)
+                        bins_epilogue_lanebin(TrueT{});
+                    else
+                        bins_epilogue_lanebin(FalseT{});
+                }
                 else
                     bins_epilogue(FalseT{}, TrueT{});
             }
