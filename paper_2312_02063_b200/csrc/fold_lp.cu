@@ -366,6 +366,7 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
         // slot r = g, its LP_WPR warps split the octets of bins (one 32-byte sector per output
         // array and lane).
         const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
+        const double pivot_q = __dmul_rn(pivot, __ddiv_rn(1.0, inv_scale));   // in units of 2^-s: exact
         const int octs = (nb + 7) >> 3;               // GEN: the last octet may be partial
         const bool vec8 = vec && !(nb & 7);
         const int r = warp / LP_WPR, wr = warp - r * LP_WPR;
@@ -400,25 +401,27 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                         S = 0;
                         c = 0;
                     }
-                    const double sq = __dmul_rn((double)S, inv_scale);
+                    const double Sd = (double)S;
                     const double cd = (double)c;
-                    fs[e] = (float)__dadd_rn(sq, __dmul_rn(cd, center));
+                    fs[e] = (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn(cd, center));
                     fc[e] = c;
                     unsigned dw = 0u;
                     if (want_norm) {
-                        // mean = sq / c through the table of correctly rounded reciprocals:
-                        // q0 = sq r, one residual correction (exact whenever the quotient is
-                        // representable, like div_by_count)
+                        // mean = S / c, in units of 2^-s (the fixed-point quantum: whatever the
+                        // flux scale, the deviations are then of order 1 .. 2^31 and fit fp32),
+                        // through the table of correctly rounded reciprocals: q0 = S r, one
+                        // residual correction (exact whenever the quotient is representable,
+                        // like div_by_count)
                         double m;
                         if (c < (unsigned)LP_RT_N) {
                             const double rc = rt[c];           // c == 0: inf, discarded below
-                            const double q0 = __dmul_rn(sq, rc);
-                            m = __fma_rn(__fma_rn(-q0, cd, sq), rc, q0);
+                            const double q0 = __dmul_rn(Sd, rc);
+                            m = __fma_rn(__fma_rn(-q0, cd, Sd), rc, q0);
                         } else {
-                            m = div_by_count_slow(sq, c);
+                            m = div_by_count_slow(Sd, c);
                         }
                         const bool nz = c > 0u;
-                        const double d = nz ? __dsub_rn(m, pivot) : 0.0;
+                        const double d = nz ? __dsub_rn(m, pivot_q) : 0.0;
                         s1 += d;
                         s2 += __dmul_rn(d, d);
                         kk += nz ? 1 : 0;
@@ -467,24 +470,26 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                     s2 += ps2[w * LP_GROUP + warp * 32 + lane];
                     kk += pkk[w * LP_GROUP + warp * 32 + lane];
                 }
-                double mu = 0.0, isd = 0.0;
+                // mean and population std of the deviations, in units of 2^-s
+                double dm = 0.0, isd = 0.0;
                 if (kk > 0) {
-                    const double dm = __ddiv_rn(s1, (double)kk);
-                    mu = __dadd_rn(pivot, dm);
+                    dm = __ddiv_rn(s1, (double)kk);
                     const double var = __dsub_rn(__ddiv_rn(s2, (double)kk), __dmul_rn(dm, dm));
                     const double sd = (var > 0.0) ? sqrt(var) : 0.0;
                     if (kk >= 2 && sd > 0.0) isd = __ddiv_rn(1.0, sd);
                 }
-                st_mu[warp * 32 + lane] = mu;
+                st_mu[warp * 32 + lane] = dm;
                 st_isd[warp * 32 + lane] = isd;
                 st_kk[warp * 32 + lane] = kk;
             }
             __syncthreads();
-            // sweep 2: out = base + (d - dm) / s from the fp32 deviations, in fp32 (d - dm over s
-            // is a z-score of a few units, base = mu + center: each rounding is 6e-8 relative
-            // against the 1e-4 bar of the normalised profile); rows cleared (same split as sweep 1)
-            const double mu = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
-            const float dmf = (float)__dsub_rn(mu, pivot), isdf = ok ? (float)isd : 0.f;
+            // sweep 2: out = base + (d - dm) / s from the fp32 deviations, in fp32 (d, dm and s in
+            // units of 2^-s; (d - dm) / s is a z-score of a few units, base = mu + center: each
+            // rounding is 6e-8 relative against the 1e-4 bar of the normalised profile); rows
+            // cleared (same split as sweep 1)
+            const double dm = st_mu[r * 32 + lane], isd = st_isd[r * 32 + lane];
+            const double mu = __dadd_rn(pivot, __dmul_rn(dm, inv_scale));      // profile mean, flux units
+            const float dmf = (float)dm, isdf = ok ? (float)isd : 0.f;
             const float basef = (ok && st_kk[r * 32 + lane] > 0) ? (float)__dadd_rn(mu, center) : 0.f;
             for (int oct = wr; oct < octs; oct += LP_WPR) {
                 float fn[8];

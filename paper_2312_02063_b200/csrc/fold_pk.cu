@@ -406,6 +406,9 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
         }
         }
         const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
+        // the bins epilogues keep deviations from the curve mean in units of 2^-s (the
+        // fixed-point quantum): of order 1 .. 2^31 whatever the flux scale, so they fit fp32
+        const double pivot_q = __dmul_rn(pivot, __ddiv_rn(1.0, inv_scale));   // exact
         const bool ok = live && valid;
 
         // The epilogues are compiled twice / four times: with and without the 32-bit side
@@ -450,15 +453,15 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                         S = 0;
                         c = 0;
                     }
-                    const double sq = __dmul_rn((double)S, inv_scale);
-                    fs[e] = (float)__dadd_rn(sq, __dmul_rn((double)c, center));
+                    const double Sd = (double)S;
+                    fs[e] = (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn((double)c, center));
                     fc[e] = c;
                     if (want_norm) {
                         // deviation of the bin mean from the curve mean, kept as fp32 in the
                         // bin's (cleared) sum word for sweep 2: NaN = empty bin
                         float df = __int_as_float(0x7fc00000);
                         if (c > 0) {
-                            const double d = __dsub_rn(pk_div_by_count(sq, c), pivot);
+                            const double d = __dsub_rn(pk_div_by_count(Sd, c), pivot_q);
                             s1 += d;
                             s2 += __dmul_rn(d, d);
                             kk += 1;
@@ -503,23 +506,23 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                             t2 += ps2[w * 32 + s * PL + tid];
                             tk += pkk[w * 32 + s * PL + tid];
                         }
-                    double mu = 0.0, isd = 0.0;
+                    // mean and population std of the deviations, in units of 2^-s
+                    double dm = 0.0, isd = 0.0;
                     if (tk > 0) {
-                        const double dm = __ddiv_rn(t1, (double)tk);
-                        mu = __dadd_rn(pivot, dm);
+                        dm = __ddiv_rn(t1, (double)tk);
                         const double var = __dsub_rn(__ddiv_rn(t2, (double)tk), __dmul_rn(dm, dm));
                         const double sdv = (var > 0.0) ? sqrt(var) : 0.0;
                         if (tk >= 2 && sdv > 0.0) isd = __ddiv_rn(1.0, sdv);
                     }
-                    st_mu[tid] = mu;
+                    st_mu[tid] = dm;
                     st_isd[tid] = isd;
                     st_kk[tid] = tk;
                 }
                 __syncthreads();
                 // sweep 2: normalised profile from the fp32 deviations (|d| is a few profile
                 // sigmas, so fp32 keeps (d - dm) / s to ~1e-6), sum words cleared
-                const double mu = st_mu[p], isd = st_isd[p];
-                const double dm = __dsub_rn(mu, pivot);
+                const double dm = st_mu[p], isd = st_isd[p];
+                const double mu = __dadd_rn(pivot, __dmul_rn(dm, inv_scale));    // profile mean, flux units
                 const double base_o = (ok && st_kk[p] > 0) ? __dadd_rn(mu, center) : 0.0;
                 for (int blk = warp; blk < nblk; blk += PK_WARPS) {
                     float fn[8];
@@ -613,7 +616,7 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                     unsigned c = (t >= 16) ? (w >> 16) : ((w & 0xffffu) - (w >> 16));
                     S = okp ? S : 0;
                     c = okp ? c : 0u;
-                    const double sq = __dmul_rn((double)S, inv_scale);
+                    const double Sd = (double)S;
                     double r, cd;
                     if (c < (unsigned)PK_RT_N) {
                         const double2 tb = rt[c];          // c == 0: {inf, 0}, discarded below
@@ -624,14 +627,15 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                         r = __ddiv_rn(1.0, cd);
                     }
                     if (w_sum && lv)
-                        *reinterpret_cast<float *>((char *)a.out_sum + po) = (float)__dadd_rn(sq, __dmul_rn(cd, center));
+                        *reinterpret_cast<float *>((char *)a.out_sum + po) =
+                            (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn(cd, center));
                     if (w_cnt && lv) *reinterpret_cast<uint32_t *>((char *)a.out_count + po) = c;
                     unsigned dw = 0u;
                     if (want_norm) {
-                        const double q0 = __dmul_rn(sq, r);
-                        const double m = __fma_rn(__fma_rn(-q0, cd, sq), r, q0);
+                        const double q0 = __dmul_rn(Sd, r);
+                        const double m = __fma_rn(__fma_rn(-q0, cd, Sd), r, q0);      // S / c, units of 2^-s
                         const bool nz = c > 0u;
-                        const double d = nz ? __dsub_rn(m, pivot) : 0.0;
+                        const double d = nz ? __dsub_rn(m, pivot_q) : 0.0;
                         s1 += d;
                         s2 += __dmul_rn(d, d);
                         kk += nz ? 1 : 0;
@@ -662,16 +666,17 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                         t2 += ps2[tid * 3 + q3];
                         tk += pkk[tid * 3 + q3];
                     }
-                    double mu = 0.0, isd = 0.0;
+                    // mean and population std of the deviations, in units of 2^-s
+                    double dm = 0.0, isd = 0.0;
                     if (tk > 0) {
-                        const double dm = __ddiv_rn(t1, (double)tk);
-                        mu = __dadd_rn(pivot, dm);
+                        dm = __ddiv_rn(t1, (double)tk);
                         const double var = __dsub_rn(__ddiv_rn(t2, (double)tk), __dmul_rn(dm, dm));
                         const double sdv = (var > 0.0) ? sqrt(var) : 0.0;
                         if (tk >= 2 && sdv > 0.0) isd = __ddiv_rn(1.0, sdv);
                     }
+                    const double mu = __dadd_rn(pivot, __dmul_rn(dm, inv_scale));   // profile mean, flux units
                     // tid is the period here, as in `ok`
-                    st_dm[tid] = (float)__dsub_rn(mu, pivot);
+                    st_dm[tid] = (float)dm;
                     st_isd[tid] = ok ? (float)isd : 0.f;
                     st_base[tid] = (ok && tk > 0) ? (float)__dadd_rn(mu, center) : 0.f;
                 }

@@ -6,6 +6,8 @@ absolute; normalised profiles within 1e-4 * max(1, |ref|) (reading R14).  For th
 config inputs (flux on the 2^-24 lattice) the fixed-point sums are exact, so the
 fp32 sums are compared bit for bit as well.
 """
+import dataclasses
+
 import numpy as np
 import pytest
 
@@ -527,3 +529,45 @@ def test_two_host_threads_on_their_own_streams(gp, ref):
     for k in range(2):
         for x, y in zip(got[k], alone[k]):
             assert torch.equal(x, y)
+
+
+@pytest.mark.parametrize("nbins", [128, 250, 256, 1024, 4096])
+def test_every_subset_of_outputs(gp, ref, nbins):
+    """The epilogues are specialised per set of requested outputs (all three, the normalised
+    profile alone, anything else): every subset gives the same arrays as the full call, and
+    the full call matches the oracle.  Several curves share t0 with their first samples
+    (zero-time samples are added to bin 0 apart from the fold)."""
+    w = workloads.config2(ncurves=3, nperiods=101)
+    w.times[w.offsets[1] + 1] = w.times[w.offsets[1]]          # two samples at t == t0
+    periods = ref.make_period_grid(w.pmin, w.pmax, w.nperiods)
+    periods[17] = np.nan
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins)
+    full = run_gpu(gp, dataclasses.replace(w, nbins=nbins), periods)
+    check(full, r, exact_sums=True)
+    for want in (("sum",), ("count",), ("norm",), ("sum", "count"), ("sum", "norm"), ("count", "norm")):
+        g = run_gpu(gp, dataclasses.replace(w, nbins=nbins), periods, want=want)
+        for k in ("sum", "count", "norm"):
+            if k in want:
+                assert np.array_equal(g[k], full[k]), (want, k)
+            else:
+                assert g[k] is None
+
+
+@pytest.mark.parametrize("nbins", [128, 256, 1024, 4096])
+def test_normalised_profile_does_not_depend_on_the_flux_scale(gp, ref, nbins):
+    """The epilogues keep fp32 deviations in units of the curve's fixed-point quantum, so a
+    curve scaled by 2^-123 (fp32 denormals: flux of order 1e-40, bin-mean deviations of order
+    2^-140, which fp32 itself would keep to 9 bits) or by 2^40 still gives the oracle's
+    normalised profile: the z-score part is scale-free, only the profile mean carries the scale."""
+    w = workloads.config2(ncurves=2, nperiods=64)
+    periods = ref.make_period_grid(w.pmin, w.pmax, w.nperiods)
+    for scale in (2.0 ** -123, 2.0 ** 40):
+        flux = (w.flux.astype(np.float64) * scale).astype(np.float32)
+        ws = dataclasses.replace(w, flux=flux, nbins=nbins)
+        g = run_gpu(gp, ws, periods)
+        r = ref.fold_batch(ws.times, ws.flux, ws.offsets, periods, nbins)
+        assert np.array_equal(g["count"], r["count"])
+        ok = np.abs(g["sum"].astype(np.float64) - r["sum64"]) <= 1e-6 * scale * np.maximum(r["count"], 1)
+        assert ok.all()
+        err = np.abs(g["norm"].astype(np.float64) - r["norm64"])
+        assert np.all(err <= 1e-4 * np.maximum(1.0, np.abs(r["norm64"])))
