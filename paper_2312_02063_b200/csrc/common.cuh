@@ -79,6 +79,10 @@ struct FoldArgs {
     float *out_mean2;             // [curve][period][nb2]
     float *out_norm2;             // [curve][period][nb2]
     unsigned *side;               // fold_pk.cu: 32-bit count overflow area, 32768 words per CTA, or NULL
+    // Non-NULL (the unfused two-tier route, api.cu): out_sum holds the sums of flux - center
+    // (small numbers: their fp32 rounding no longer costs the 6e-8 of an uncentred flux near 1)
+    // and the curve's center goes to center_out[curve] for the merge kernel to add back.
+    double *center_out;
     unsigned long long *stats;    // device counters (DeviceInfo::stats), or NULL
 };
 
@@ -213,7 +217,8 @@ cudaError_t merge_init_device();
 cudaError_t launch_normalize(const float *sum, const uint32_t *count, long long nprofiles,
                              int nbins, float *out, cudaStream_t st);
 cudaError_t launch_merge(const float *sum, const uint32_t *count, long long nprofiles, int nb1,
-                         int nb2, float *out_mean, float *out_norm, cudaStream_t st);
+                         int nb2, float *out_mean, float *out_norm, const double *offset,
+                         cudaStream_t st);
 cudaError_t launch_grid(double pmin, double pmax, long long nperiods, int mode_flags,
                         double *out, cudaStream_t st);
 cudaError_t measure_peaks(double *out_host, cudaStream_t st);

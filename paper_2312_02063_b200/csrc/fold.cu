@@ -50,7 +50,9 @@ fold_generic_kernel(FoldArgs a, long long nitems)
         __syncthreads();
         if (tid < 32) {
             const long long row = (curve * a.nperiods + j) * (long long)nb;
-            emit_profile(R, nb, tid, m.inv_scale, m.center, false,
+            if (a.center_out && j == 0 && tid == 0) a.center_out[curve] = m.center;
+            // centred sums (FoldArgs::center_out) come without a normalised profile (api.cu)
+            emit_profile(R, nb, tid, m.inv_scale, a.center_out ? 0.0 : m.center, false,
                          a.out_sum ? a.out_sum + row : nullptr,
                          a.out_count ? a.out_count + row : nullptr,
                          a.out_norm ? a.out_norm + row : nullptr);

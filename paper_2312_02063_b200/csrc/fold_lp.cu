@@ -367,6 +367,8 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
         // array and lane).
         const double inv_scale = cm.inv_scale, center = cm.center, pivot = cm.pivot;
         const double pivot_q = __dmul_rn(pivot, __ddiv_rn(1.0, inv_scale));   // in units of 2^-s: exact
+        const double center_s = a.center_out ? 0.0 : center;       // FoldArgs::center_out: centred sums
+        if (a.center_out && p0 == 0 && tid == 0) a.center_out[curve] = center;
         const int octs = (nb + 7) >> 3;               // GEN: the last octet may be partial
         const bool vec8 = vec && !(nb & 7);
         const int r = warp / LP_WPR, wr = warp - r * LP_WPR;
@@ -403,7 +405,7 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                     }
                     const double Sd = (double)S;
                     const double cd = (double)c;
-                    fs[e] = (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn(cd, center));
+                    fs[e] = (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn(cd, center_s));
                     fc[e] = c;
                     unsigned dw = 0u;
                     if (want_norm) {

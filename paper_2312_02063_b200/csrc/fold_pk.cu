@@ -409,6 +409,8 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
         // the bins epilogues keep deviations from the curve mean in units of 2^-s (the
         // fixed-point quantum): of order 1 .. 2^31 whatever the flux scale, so they fit fp32
         const double pivot_q = __dmul_rn(pivot, __ddiv_rn(1.0, inv_scale));   // exact
+        const double center_s = a.center_out ? 0.0 : center;       // FoldArgs::center_out: centred sums
+        if (a.center_out && p0 == 0 && tid == 0) a.center_out[curve] = center;
         const bool ok = live && valid;
 
         // The epilogues are compiled twice / four times: with and without the 32-bit side
@@ -454,7 +456,7 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                         c = 0;
                     }
                     const double Sd = (double)S;
-                    fs[e] = (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn((double)c, center));
+                    fs[e] = (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn((double)c, center_s));
                     fc[e] = c;
                     if (want_norm) {
                         // deviation of the bin mean from the curve mean, kept as fp32 in the
@@ -628,7 +630,7 @@ __device__ __forceinline__ void fold_pk_body(const FoldArgs &a, long long ngroup
                     }
                     if (w_sum && lv)
                         *reinterpret_cast<float *>((char *)a.out_sum + po) =
-                            (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn(cd, center));
+                            (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn(cd, center_s));
                     if (w_cnt && lv) *reinterpret_cast<uint32_t *>((char *)a.out_count + po) = c;
                     unsigned dw = 0u;
                     if (want_norm) {

@@ -23,8 +23,11 @@ constexpr int MERGE_SEG = 512;       // fine bins staged per pass (per warp: 4.3
 __global__ void __launch_bounds__(MERGE_THREADS)
 merge_equal_count_kernel(const float *__restrict__ sum, const uint32_t *__restrict__ count,
                          long long nprofiles, int nb1, int nb2, float *__restrict__ out_mean,
-                         float *__restrict__ out_norm)
+                         float *__restrict__ out_norm, const double *__restrict__ offset)
 {
+    // a constant the sums were taken relative to (the unfused route of gpfc_fold_two_tier passes
+    // the curve's center): every output bin holds exactly N / nb2 points, so its mean shifts by it
+    const double off = offset ? *offset : 0.0;
     extern __shared__ __align__(16) unsigned char merge_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nwarps = blockDim.x >> 5;
@@ -155,7 +158,7 @@ merge_equal_count_kernel(const float *__restrict__ sum, const uint32_t *__restri
         double acc = 0.0;
         for (int bb = lane; bb < nb2; bb += 32) {
             const double m = __ddiv_rn(__dsub_rn(scum[bb + 1], scum[bb]), per);
-            if (out_mean) out_mean[prof * nb2 + bb] = (float)m;
+            if (out_mean) out_mean[prof * nb2 + bb] = (float)__dadd_rn(m, off);
             acc += m;
         }
         if (out_norm) {
@@ -171,7 +174,8 @@ merge_equal_count_kernel(const float *__restrict__ sum, const uint32_t *__restri
             const bool flat = (nb2 < 2) || !(sd > 0.0);
             for (int bb = lane; bb < nb2; bb += 32) {
                 const double m = __ddiv_rn(__dsub_rn(scum[bb + 1], scum[bb]), per);
-                const double o = flat ? mu : __dadd_rn(mu, __ddiv_rn(__dsub_rn(m, mu), sd));
+                const double o = flat ? __dadd_rn(mu, off)
+                                      : __dadd_rn(__dadd_rn(mu, off), __ddiv_rn(__dsub_rn(m, mu), sd));
                 out_norm[prof * nb2 + bb] = (float)o;
             }
         }
@@ -188,7 +192,8 @@ cudaError_t merge_init_device()
 }
 
 cudaError_t launch_merge(const float *sum, const uint32_t *count, long long nprofiles, int nb1,
-                         int nb2, float *out_mean, float *out_norm, cudaStream_t st)
+                         int nb2, float *out_mean, float *out_norm, const double *offset,
+                         cudaStream_t st)
 {
     if (nprofiles <= 0) return cudaSuccess;
     int warps = MERGE_THREADS / 32;
@@ -199,7 +204,7 @@ cudaError_t launch_merge(const float *sum, const uint32_t *count, long long npro
     if (blocks > 148LL * 16) blocks = 148LL * 16;
     size_t smem = (size_t)warps * per_warp;
     merge_equal_count_kernel<<<(unsigned)blocks, warps * 32, smem, st>>>(
-        sum, count, nprofiles, nb1, nb2, out_mean, out_norm);
+        sum, count, nprofiles, nb1, nb2, out_mean, out_norm, offset);
     note_launch();
     return cudaGetLastError();
 }

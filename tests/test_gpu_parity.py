@@ -571,3 +571,17 @@ def test_normalised_profile_does_not_depend_on_the_flux_scale(gp, ref, nbins):
         assert ok.all()
         err = np.abs(g["norm"].astype(np.float64) - r["norm64"])
         assert np.all(err <= 1e-4 * np.maximum(1.0, np.abs(r["norm64"])))
+
+
+@pytest.mark.parametrize("nbins,nperiods", [(256, 14500), (100, 14500), (128, 96 * 148 + 1), (256, 96 * 148)])
+def test_item_counts_around_one_wave(gp, ref, nbins, nperiods):
+    """One curve over a few more than 148 work items of 96 periods (a second, nearly empty
+    wave of the persistent grid), a last group of a single period, exactly 148 items."""
+    w = workloads.config1(nperiods=8)
+    n = 3000
+    periods = ref.make_period_grid(0.2, 1.0, nperiods)
+    periods[[5, nperiods - 97]] = np.nan
+    ws = dataclasses.replace(w, times=w.times[:n], flux=w.flux[:n], offsets=np.array([0, n], np.int64), nbins=nbins)
+    g = run_gpu(gp, ws, periods)
+    r = ref.fold_batch(ws.times, ws.flux, ws.offsets, periods, nbins)
+    check(g, r, exact_sums=True)

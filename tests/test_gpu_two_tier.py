@@ -200,3 +200,46 @@ def test_two_tier_unfused_fallback(gp, ref):
     check_fused(gp, ref, w.times, w.flux, periods, 4096, 1024)
     check_fused(gp, ref, w.times, w.flux, periods, 4096, 300)
     assert gp.gpfc_path_counters()["unfused_two_tier_calls"] == 4
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_fused_two_tier_fuzz(gp, ref, seed):
+    """Seeded random cases of the whole two-tier fold: batch of 1-3 curves (regular cadence with
+    drops, or irregular times; flux off the lattice, any scale), 1-40 periods, (nb1, nb2) from
+    the fused and the unfused pairs, optional per-curve t0."""
+    rng = np.random.default_rng([105, 111, seed])
+    nb1 = int(rng.choice([1024, 2048, 4096]))
+    nb2 = int(rng.choice([1, 2, 7, 32, 64, 100, 128, 200, 256, 300]))
+    nc = int(rng.integers(1, 4))
+    scale = float(2.0 ** rng.integers(-20, 6))
+    ts, fs, off = [], [], [0]
+    for _ in range(nc):
+        n = int(rng.choice([0, 1, 3, 40, int(rng.integers(100, 5000))]))
+        if rng.random() < 0.5:
+            t = np.cumsum(1 + (rng.random(n) < 0.05)) * workloads.KEPLER_CADENCE_D
+        else:
+            t = np.sort(rng.uniform(0.0, 60.0, n))
+        ts.append(t)
+        fs.append(((1.0 + rng.normal(0.0, 1e-3, n)) * scale).astype(np.float32))
+        off.append(off[-1] + n)
+    times, flux = np.concatenate(ts), np.concatenate(fs)
+    periods = np.sort(rng.uniform(0.2, float(rng.choice([1.0, 10.0])), int(rng.integers(1, 41))))
+    t0 = rng.uniform(-1.0, 1.0, nc) if rng.random() < 0.5 else None
+    off = np.asarray(off, np.int64)
+    # check_fused's absolute 1e-6 bar is for relative flux: scale the curves back for it
+    m, _ = check_fused(gp, ref, times, (flux.astype(np.float64) / scale).astype(np.float32), periods,
+                       nb1, nb2, t0=t0, offsets=off, lattice=False)
+    assert np.all(np.isfinite(m))
+    # and at the drawn scale: merged means relative to the profile's magnitude
+    mean, norm = gp.gpfc_fold_two_tier(dev(times), dev(flux), dev(off), dev(periods), nb1, nb2,
+                                       t0=None if t0 is None else dev(t0))
+    torch.cuda.synchronize()
+    for c in range(nc):
+        a, b = int(off[c]), int(off[c + 1])
+        omean, onorm, has = oracle_two_tier(ref, times[a:b], flux[a:b], periods, nb1, nb2,
+                                            0.0 if t0 is None else float(t0[c]))
+        assert np.all(np.abs(mean[c].cpu().numpy() - omean) <= 1e-6 * scale * 2.0)
+        sd = omean.std(axis=-1)
+        defined = sd >= 1e-9 * np.abs(omean).max(axis=-1)
+        err = np.abs(norm[c].cpu().numpy() - onorm)
+        assert np.all(err[defined] <= 1e-4 * np.maximum(1.0, np.abs(onorm[defined])))
