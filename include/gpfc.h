@@ -163,7 +163,10 @@ int gpfc_normalize(const float *sum, const uint32_t *count, int64_t nprofiles, i
  *   out_mean     device fp32 [nprofiles][nb2]  mean flux of each final bin   (may be NULL)
  *   out_norm     device fp32 [nprofiles][nb2]  the same profile noise-normalised as in
  *                gpfc_normalize (every final bin counts as non-empty)        (may be NULL)
- * A profile without points gives zeros.  Arithmetic in fp64.
+ * A profile without points gives zeros.  Arithmetic in fp64; the input sums are fp32, so the
+ * merged means carry their rounding (6e-8 relative to the flux level: for a normalised profile
+ * of an UNCENTRED relative flux near 1 with a spread of a few 1e-4 that is ~1e-4 of its unit;
+ * median-subtracted flux, as gpfc_fold asks for, or gpfc_fold_two_tier do not have this limit).
  */
 int gpfc_merge_equal_count(const float *sum, const uint32_t *count, int64_t nprofiles, int nb1,
                            int nb2, float *out_mean, float *out_norm);
@@ -203,7 +206,8 @@ int gpfc_fold_batch(const double *times, const float *flux, const int64_t *offse
  * For nb1 in {1024, 2048, 4096} and nb2 <= nb1 / 16 (256 for nb1 = 4096, the paper's pair)
  * fold and merge are ONE kernel: the intermediary profile stays in shared memory and the merge
  * reads the exact integer sums.  Any other (nb1, nb2) folds into a temporary intermediary
- * profile (stream-ordered allocation, <= 256 MB) and runs gpfc_merge_equal_count on it.
+ * profile (stream-ordered allocation, <= 256 MB; fp32 sums taken relative to the curve's
+ * internal center, which the merge adds back) and runs the kernel of gpfc_merge_equal_count.
  * A period that is not finite-positive, or a curve without valid samples, gives zeros.
  */
 int gpfc_fold_two_tier(const double *times, const float *flux, const int64_t *offsets,
