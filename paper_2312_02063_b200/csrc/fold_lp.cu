@@ -1,6 +1,7 @@
-// fold_lp_kernel: the "lane = period" fold for power-of-two nbins in [32, 256]
+// fold_lp_kernel: the "lane = period" fold for every nbins <= 256 (powers of two from 32 at 256
+// rows, fold_lp_kernel<false>; anything else one row per bin, fold_lp_kernel<true>)
 // (PAPER.md:111 steps 1-3 and 5, noise normalisation :63 fused into the epilogue).
-// DESIGN.md "Kernel design" has the full derivation; in short:
+// DESIGN.md 6.1 has the full derivation; in short:
 //
 // * One persistent CTA per SM.  A work item is (curve, group of 32*R consecutive trial
 //   periods).  Lane l of EVERY warp owns the R periods p0 + r*32 + l; the warps split
@@ -26,8 +27,12 @@
 //   sample against the exact formula and corrected with compensating atomics.
 // * nbins < 256 folds at 256 rows and merges 256 / nbins adjacent rows at write-out
 //   (exact: floor(phi * 256) >> k == floor(phi * (256 >> k))).
+// * The fold loop is unrolled 8x (32 samples per iteration); per sample the three ATOMS.ADD
+//   come before the three ATOMS.POPC.INC (fewer replays in the atomic unit).
 // * Epilogue: lane l walks ITS periods' rows (conflict-free), so mean / std need no
-//   cross-lane reduction; every lane writes 32-byte sectors (8 bins) of its own rows.
+//   cross-lane reduction; every lane writes 32-byte sectors (8 bins) of its own rows.  Bin
+//   means through a shared-memory table of correctly rounded reciprocals; deviations from the
+//   curve mean kept as fp32 in units of the fixed-point quantum; second sweep in fp32.
 #include "common.cuh"
 
 namespace gpfc {

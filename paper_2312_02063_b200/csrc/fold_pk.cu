@@ -11,15 +11,19 @@
 //   high half-word counts row k + ROWS/2 alone.  The bank of a word is (row mod SL) * PL + p:
 //   one conflict-free wavefront per warp-wide atomic when SL = 1; for SL > 1 two slots collide
 //   when their rows agree mod SL (hardware replays, correctness is not affected).
-//   A half-word cannot overflow while at most 65,535 samples have been added, so the counts
-//   are flushed to a 32-bit side array in global memory (one per CTA, L2-resident) every
-//   65,408 samples: curves of any length stay on this kernel (the paper's Kepler curves have
-//   up to 70,000 epochs).
+//   A half-word cannot overflow while at most 65,535 samples have been added.  Longer curves
+//   (the paper's Kepler curves have up to 70,000 epochs) are folded without
+//   a flush first and checked (the low half-words of a period add up to n_valid iff none
+//   wrapped); only if one did is the item folded again in segments of 65,408 samples with the
+//   counts flushed to a 32-bit side array in global memory (one per CTA, L2-resident) between.
 // * Phase math, guard band and exact re-check: as in fold_lp.cu (one DFMA.RM per point-period,
 //   m = RD(v rp + C), row = bits of the high word, fraction = the low word; a tile whose
-//   smallest fraction is inside the guard band is re-checked against the exact formula).
+//   smallest fraction is inside the guard band is re-checked against the exact formula, by
+//   the whole warp, 32 samples at a time for every flagged lane).  Fold loop unrolled 8x.
 // * Epilogue, one of
 //   (1) bins: sums / counts (/ normalised profile) of nbins = ROWS >> k bins, written per lane;
+//   (1b) bins at ROWS = nbins = 1024 (config 3): the row vectors are permuted in place so that
+//       a warp walks the bins of one period with lane = bin, and every store is a full line;
 //   (2) merge: the nbins intermediary bins are merged left to right into nb2 bins of equal
 //       count (boundary bins split pro rata, R18) straight from the exact integer
 //       sums in shared memory -- the intermediary profile never reaches HBM -- then the mean

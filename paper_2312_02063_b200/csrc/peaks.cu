@@ -119,9 +119,10 @@ __global__ void __launch_bounds__(1024, 1) peak_fp64_kernel(int iters, double se
     if (acc == 0xdeadbeefu) sink[0] = (double)acc;
 }
 
-// [2] the inner loop of fold_lp_kernel<0> alone (lane = period, 3 periods per lane, 8-byte
+// [2] the inner loop of fold_lp_kernel<false> alone (lane = period, 3 periods per lane, 8-byte
 // sample records broadcast from shared memory, DFMA.RM + PRMT + VIMNMX3 + ATOMS.ADD +
-// ATOMS.POPC.INC per point-period): no global loads, tile set-up, epilogue or barriers.
+// ATOMS.POPC.INC per point-period, 32 samples per iteration): no global loads, tile set-up,
+// epilogue or barriers.
 template <int IMM>
 __device__ __forceinline__ void pk_red_add(unsigned addr, int v)
 {
@@ -152,23 +153,32 @@ __global__ void __launch_bounds__(768, 1) peak_loop_kernel(int nsamples, double 
         C[r] = 1048576.0 + (double)((r * 97 + lane * 13) & 255) + 0.375;
     }
     unsigned gmin = 0xffffffffu;
-    for (int s0 = warp * 4; s0 < nsamples; s0 += 4 * (blockDim.x >> 5)) {
-        const int4 ra = rec[(s0 >> 1) & 31], rb = rec[((s0 >> 1) + 1) & 31];
-        const unsigned iv[4] = {(unsigned)ra.x + s0, (unsigned)ra.z + s0, (unsigned)rb.x + s0,
-                                (unsigned)rb.z + s0};
-        const int q[4] = {ra.y, ra.w, rb.y, rb.w};
+    // as fold_lp.cu's fold_granule: 32 samples per iteration, per sample the three sums before
+    // the three counts
+    for (int s0 = warp * 32; s0 < nsamples; s0 += 32 * (blockDim.x >> 5)) {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const double v = (double)iv[k];
+        for (int g = 0; g < 8; ++g) {
+            const int4 ra = rec[((s0 >> 1) + 2 * g) & 31], rb = rec[((s0 >> 1) + 2 * g + 1) & 31];
+            const unsigned iv[4] = {(unsigned)ra.x + s0, (unsigned)ra.z + s0, (unsigned)rb.x + s0,
+                                    (unsigned)rb.z + s0};
+            const int q[4] = {ra.y, ra.w, rb.y, rb.w};
 #pragma unroll
-            for (int r = 0; r < 3; ++r) {
-                double m = __fma_rd(v, rp[r], C[r]);
-                unsigned lo = (unsigned)__double2loint(m), hi = (unsigned)__double2hiint(m);
-                unsigned addr = __byte_perm(lane4, hi, 0x3240) + sbase;
-                gmin = min(gmin, lo);
-                if (r == 0) { pk_red_add<0>(addr, q[k]); pk_red_inc<128>(addr); }
-                if (r == 1) { pk_red_add<65536>(addr, q[k]); pk_red_inc<65536 + 128>(addr); }
-                if (r == 2) { pk_red_add<131072>(addr, q[k]); pk_red_inc<131072 + 128>(addr); }
+            for (int k = 0; k < 4; ++k) {
+                const double v = (double)iv[k];
+                unsigned addr[3];
+#pragma unroll
+                for (int r = 0; r < 3; ++r) {
+                    double m = __fma_rd(v, rp[r], C[r]);
+                    unsigned lo = (unsigned)__double2loint(m), hi = (unsigned)__double2hiint(m);
+                    addr[r] = __byte_perm(lane4, hi, 0x3240) + sbase;
+                    gmin = min(gmin, lo);
+                }
+                pk_red_add<0>(addr[0], q[k]);
+                pk_red_add<65536>(addr[1], q[k]);
+                pk_red_add<131072>(addr[2], q[k]);
+                pk_red_inc<128>(addr[0]);
+                pk_red_inc<65536 + 128>(addr[1]);
+                pk_red_inc<131072 + 128>(addr[2]);
             }
         }
     }
