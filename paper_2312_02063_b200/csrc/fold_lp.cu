@@ -69,6 +69,15 @@ static_assert(GPFC_TILE == 2 * LP_GRAN, "half-tile work units are one staging gr
 static_assert(LP_WARPS * LP_GRAN * 8 <= LP_MU_OFF - LP_STAGE_OFF, "staging fits in the scratch");
 static_assert(LP_WARPS % LP_R == 0, "warps per period slot");
 
+template <int N>
+struct LpInt {
+    static constexpr int value = N;
+};
+template <bool B>
+struct LpBool {
+    static constexpr bool value = B;
+};
+
 // shared-memory reductions with an immediate offset: ATOMS.ADD / ATOMS.POPC.INC [R + UR + imm].
 // `addr` carries the shared-window address of the histogram (__cvta_generic_to_shared), which
 // ptxas keeps in a uniform register: the window base is never assumed.
@@ -390,15 +399,22 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
             // one-pass moments of d (exactly zero for a flat profile).
             double s1 = 0.0, s2 = 0.0;
             int kk = 0;
+            // compiled per (rows per bin, sums / counts wanted or not): the common cases carry
+            // no dead arithmetic and no run-time row loop
+            auto sweep1 = [&](auto m_c, auto ws_c) {
+            constexpr int MC = decltype(m_c)::value;           // rows per bin; 0: M, at run time
+            constexpr bool WS = decltype(ws_c)::value;         // out_sum or out_count wanted
+            const int MM = MC ? MC : M;
             for (int oct = wr; oct < octs; oct += LP_WPR) {
                 float fs[8];
                 unsigned fc[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    unsigned *h0 = Hr + (oct * 8 + e) * M * 64;
+                    unsigned *h0 = Hr + (oct * 8 + e) * MM * 64;
                     int S = (int)h0[0];
                     unsigned c = h0[32];
-                    for (int jj = 1; jj < M; ++jj) {
+#pragma unroll
+                    for (int jj = 1; jj < MM; ++jj) {
                         S += (int)h0[jj * 64];
                         c += h0[jj * 64 + 32];
                         h0[jj * 64] = 0u;
@@ -410,8 +426,10 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                     }
                     const double Sd = (double)S;
                     const double cd = (double)c;
-                    fs[e] = (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn(cd, center_s));
-                    fc[e] = c;
+                    if constexpr (WS) {
+                        fs[e] = (float)__dadd_rn(__dmul_rn(Sd, inv_scale), __dmul_rn(cd, center_s));
+                        fc[e] = c;
+                    }
                     unsigned dw = 0u;
                     if (want_norm) {
                         // mean = S / c, in units of 2^-s (the fixed-point quantum: whatever the
@@ -437,7 +455,7 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                     h0[0] = dw;
                     h0[32] = 0u;
                 }
-                if (live) {
+                if (WS && live) {
                     const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
                     if (vec8) {
                         if (a.out_sum) {
@@ -460,6 +478,21 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                         }
                     }
                 }
+            }
+            };
+            const bool ws = a.out_sum != nullptr || a.out_count != nullptr;
+            if (M == 1) {
+                if (ws)
+                    sweep1(LpInt<1>{}, LpBool<true>{});
+                else
+                    sweep1(LpInt<1>{}, LpBool<false>{});
+            } else if (M == 2) {
+                if (ws)
+                    sweep1(LpInt<2>{}, LpBool<true>{});
+                else
+                    sweep1(LpInt<2>{}, LpBool<false>{});
+            } else {
+                sweep1(LpInt<0>{}, LpBool<true>{});
             }
             if (want_norm) {
                 ps1[wr * LP_GROUP + r * 32 + lane] = s1;
@@ -498,11 +531,14 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
             const double mu = __dadd_rn(pivot, __dmul_rn(dm, inv_scale));      // profile mean, flux units
             const float dmf = (float)dm, isdf = ok ? (float)isd : 0.f;
             const float basef = (ok && st_kk[r * 32 + lane] > 0) ? (float)__dadd_rn(mu, center) : 0.f;
+            auto sweep2 = [&](auto m_c) {
+            constexpr int MC = decltype(m_c)::value;           // rows per bin; 0: M, at run time
+            const int MM = MC ? MC : M;
             for (int oct = wr; oct < octs; oct += LP_WPR) {
                 float fn[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    unsigned *h0 = Hr + (oct * 8 + e) * M * 64;
+                    unsigned *h0 = Hr + (oct * 8 + e) * MM * 64;
                     const float df = __uint_as_float(h0[0]);
                     h0[0] = 0u;
                     // NaN (empty bin) or s == 0: the profile mean
@@ -522,6 +558,13 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                     }
                 }
             }
+            };
+            if (M == 1)
+                sweep2(LpInt<1>{});
+            else if (M == 2)
+                sweep2(LpInt<2>{});
+            else
+                sweep2(LpInt<0>{});
         }
         if (tid == 0) *ctr = 0;
         __syncthreads();   // B: H is zero again, tile counter reset
