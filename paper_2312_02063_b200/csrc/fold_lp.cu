@@ -455,7 +455,8 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                     h0[0] = dw;
                     h0[32] = 0u;
                 }
-                if (WS && live) {
+                if constexpr (WS) {
+                if (live) {
                     const long long off = ((curve * a.nperiods + j) * nb) + oct * 8;
                     if (vec8) {
                         if (a.out_sum) {
@@ -477,6 +478,7 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
                             if (a.out_count) a.out_count[off + e] = fc[e];
                         }
                     }
+                }
                 }
             }
             };
