@@ -70,6 +70,9 @@ typedef enum {
 } gpfc_status;
 
 #define GPFC_MAX_NBINS 4096
+/* limits of gpfc_fold_noalloc (its scratch is a static device array sized for them) */
+#define GPFC_NOALLOC_MAX_SAMPLES 131072
+#define GPFC_NOALLOC_MAX_PERIODS 262144
 
 /* gpfc_make_period_grid mode_flags: spacing | endpoint */
 enum { GPFC_GRID_UNIFORM_FREQUENCY = 0, GPFC_GRID_UNIFORM_PERIOD = 1 };
@@ -144,6 +147,28 @@ double gpfc_n_sample(double n_o, double t_window, double l_width);
 int gpfc_fold(const double *times, const float *flux, int64_t n,
               const double *periods, int64_t nperiods, int nbins, double t0,
               float *out_sum, uint32_t *out_count);
+
+/*
+ * gpfc_fold plus the fused noise normalisation (PAPER.md:111 "First" to "Lastly", :63), for
+ * callers that must not allocate: code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc.  This call allocates NOTHING, with or without gpfc_set_workspace: no
+ * cudaMalloc / cudaMallocAsync / cudaFree, no event creation (gpfc_profile does not time it).
+ * Its scratch (valid samples as fixed-point records, per-period reciprocals) is a static device
+ * array inside the library: 4.8 MB that every GPU which loads the library holds until exit.
+ * Arguments as gpfc_fold; out_norm device fp32 [nperiods][nbins] (may be NULL) as out_norm of
+ * gpfc_fold_batch.  Asynchronous on the thread's stream like every device-pointer call.
+ * Limits (GPFC_ERR_UNSUPPORTED with a message beyond them, nothing is launched):
+ *   n <= GPFC_NOALLOC_MAX_SAMPLES (131072), nperiods <= GPFC_NOALLOC_MAX_PERIODS (262144), and
+ *   n <= 65408 when nbins is 512, 1024, 2048 or 4096 (longer curves need the count overflow
+ *   area of that kernel, which is not part of the static scratch).
+ * All calls, from every host thread and stream, share the one array of their device: two calls
+ * whose kernels overlap on the GPU race (wrong results, no error).  Issue them on one stream, or
+ * order them with events.  The array keeps the previous call's contents; nothing in it has to
+ * start at zero (the prepass rewrites every word the fold reads), so nothing is cleared.
+ */
+int gpfc_fold_noalloc(const double *times, const float *flux, int64_t n,
+                      const double *periods, int64_t nperiods, int nbins, double t0,
+                      float *out_sum, uint32_t *out_count, float *out_norm);
 
 /*
  * Step 5 + noise normalisation of nprofiles folded profiles (PAPER.md:111

@@ -29,7 +29,7 @@ EXPORTS = [
     "gpfc_normalize", "gpfc_fold_batch", "gpfc_make_period_grid_host",
     "gpfc_fold_batch_host", "gpfc_measure_peaks", "gpfc_profile", "gpfc_profile_read",
     "gpfc_merge_equal_count", "gpfc_init", "gpfc_fold_two_tier", "gpfc_path_counters",
-    "gpfc_lc_params_default", "gpfc_make_light_curves", "gpfc_fold_stream",
+    "gpfc_lc_params_default", "gpfc_make_light_curves", "gpfc_fold_stream", "gpfc_fold_noalloc",
 ]
 OUT_SUM, OUT_COUNT, OUT_NORM = 1, 2, 4
 
@@ -95,6 +95,7 @@ def lib() -> ctypes.CDLL:
     L.gpfc_n_sample.restype = f64
     L.gpfc_n_sample.argtypes = [f64, f64, f64]
     L.gpfc_fold.argtypes = [vp, vp, i64, vp, i64, i32, f64, vp, vp]
+    L.gpfc_fold_noalloc.argtypes = [vp, vp, i64, vp, i64, i32, f64, vp, vp, vp]
     L.gpfc_normalize.argtypes = [vp, vp, i64, i32, vp]
     fb = [vp, vp, vp, i64, i64, vp, i64, i32, vp, vp, vp, vp]
     L.gpfc_fold_batch.argtypes = fb
@@ -200,6 +201,20 @@ def gpfc_fold(times, flux, periods, nbins, t0=0.0, out_sum=None, out_count=None)
                            _dptr(out_sum, torch.float32, "out_sum"),
                            _dptr(out_count, torch.int32, "out_count")), "gpfc_fold")
     return out_sum, out_count
+
+
+def gpfc_fold_noalloc(times, flux, periods, nbins, t0, out_sum, out_count, out_norm):
+    """gpfc_fold + fused normalisation on the library's static scratch: allocates nothing, so
+    the caller passes every output it wants (None = not wanted); see include/gpfc.h for the
+    size limits and the rule that overlapping calls race."""
+    n, npd = times.numel(), periods.numel()
+    _use_current_stream()
+    _check(lib().gpfc_fold_noalloc(
+        _dptr(times, torch.float64, "times"), _dptr(flux, torch.float32, "flux"), n,
+        _dptr(periods, torch.float64, "periods"), npd, int(nbins), float(t0),
+        _dptr(out_sum, torch.float32, "out_sum"), _dptr(out_count, torch.int32, "out_count"),
+        _dptr(out_norm, torch.float32, "out_norm")), "gpfc_fold_noalloc")
+    return out_sum, out_count, out_norm
 
 
 def gpfc_normalize(sum_, count, out_norm=None):

@@ -9,6 +9,23 @@
 
 #include "common.cuh"
 
+// ---- gpfc_fold_noalloc: the scratch of one single-curve fold, held by the library itself.
+// Every GPU that loads the library holds these GPFC_NOALLOC_BYTES (4.8 MB) until exit.  In host
+// code the array's name is only a stand-in for the symbol: the device address comes from
+// cudaGetSymbolAddress (noalloc_scratch_ptr below), once per device with that device current.
+constexpr int64_t GPFC_NOALLOC_SAMPLES = GPFC_NOALLOC_MAX_SAMPLES;
+constexpr int64_t GPFC_NOALLOC_PERIODS = GPFC_NOALLOC_MAX_PERIODS;
+constexpr size_t noalloc_up(size_t x) { return (x + 255) & ~(size_t)255; }
+constexpr size_t GPFC_NOALLOC_BYTES =          // the terms of scratch_bytes(1, n, np, 0) below
+    noalloc_up((size_t)GPFC_NOALLOC_SAMPLES * sizeof(double)) +
+    noalloc_up((size_t)GPFC_NOALLOC_SAMPLES * sizeof(int)) +
+    noalloc_up(((size_t)GPFC_NOALLOC_SAMPLES + 3) * sizeof(int2)) +
+    noalloc_up(((size_t)GPFC_NOALLOC_SAMPLES / gpfc::GPFC_TILE + 2) * sizeof(gpfc::TileInfo)) +
+    noalloc_up(sizeof(gpfc::CurveMeta)) +
+    noalloc_up((size_t)GPFC_NOALLOC_PERIODS * sizeof(double)) +
+    noalloc_up(2 * sizeof(int64_t)) + noalloc_up(gpfc::PREP_PART_BYTES) + 256;
+static __device__ __align__(256) unsigned char gpfc_noalloc_scratch[GPFC_NOALLOC_BYTES];
+
 namespace {
 
 struct ThreadState {
@@ -245,6 +262,29 @@ int check_bins(int nb)
     return GPFC_OK;
 }
 
+// Device address of gpfc_noalloc_scratch on the current device: asked for once per device, with
+// that device current (a symbol has one address per device); no allocation.
+void *g_noalloc_ptr[MAX_DEVICES];
+std::mutex g_noalloc_mutex;
+
+cudaError_t noalloc_scratch_ptr(void **out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, gpfc_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return cudaSuccess;
+}
+
 }  // namespace
 
 extern "C" {
@@ -376,6 +416,49 @@ int gpfc_fold(const double *times, const float *flux, int64_t n, const double *p
     o.sum = out_sum;
     o.count = out_count;
     return fold_device(times, flux, nullptr, 1, n, periods, nperiods, nbins, nullptr, t0, o);
+}
+
+int gpfc_fold_noalloc(const double *times, const float *flux, int64_t n, const double *periods,
+                      int64_t nperiods, int nbins, double t0, float *out_sum,
+                      uint32_t *out_count, float *out_norm)
+{
+    if (n < 0 || nperiods < 0) return fail(GPFC_ERR_INVALID_ARG, "negative size%s");
+    if (n > GPFC_NOALLOC_SAMPLES)
+        return fail(GPFC_ERR_UNSUPPORTED, "gpfc_fold_noalloc: more than GPFC_NOALLOC_MAX_SAMPLES "
+                                          "(131072) samples%s");
+    if (nperiods > GPFC_NOALLOC_PERIODS)
+        return fail(GPFC_ERR_UNSUPPORTED, "gpfc_fold_noalloc: more than GPFC_NOALLOC_MAX_PERIODS "
+                                          "(262144) periods%s");
+    if (check_bins(nbins) != GPFC_OK) return GPFC_ERR_UNSUPPORTED;
+    const gpfc::DeviceInfo *di = nullptr;
+    cudaError_t e = gpfc::device_info(&di);          // kernel attributes, SM count: no allocation
+    if (e != cudaSuccess) return cuda_fail(e, "device initialisation");
+    if (side_bytes_for(n, nbins, di->num_sms) != 0)
+        return fail(GPFC_ERR_UNSUPPORTED, "gpfc_fold_noalloc: nbins >= 512 takes at most 65408 samples "
+                                          "(the count overflow area is not part of the static scratch)%s");
+    if (scratch_bytes(1, n, nperiods, 0) > GPFC_NOALLOC_BYTES)
+        return fail(GPFC_ERR_WORKSPACE, "gpfc_fold_noalloc: static scratch too small%s");
+    void *scratch = nullptr;
+    e = noalloc_scratch_ptr(&scratch);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(gpfc_noalloc_scratch)");
+    // The fold itself is the library's one device path, run on the static scratch as its
+    // workspace for this call (it allocates only when the workspace is too small, which was
+    // ruled out above) and without the profiling events (cudaEventCreate) of gpfc_profile.
+    void *const ws0 = g_ts.ws;
+    const size_t wsb0 = g_ts.ws_bytes;
+    const bool prof0 = g_ts.profiling;
+    g_ts.ws = scratch;
+    g_ts.ws_bytes = GPFC_NOALLOC_BYTES;
+    g_ts.profiling = false;
+    FoldOut o;
+    o.sum = out_sum;
+    o.count = out_count;
+    o.norm = out_norm;
+    const int rc = fold_device(times, flux, nullptr, 1, n, periods, nperiods, nbins, nullptr, t0, o);
+    g_ts.ws = ws0;
+    g_ts.ws_bytes = wsb0;
+    g_ts.profiling = prof0;
+    return rc;
 }
 
 int gpfc_normalize(const float *sum, const uint32_t *count, int64_t nprofiles, int nbins,
