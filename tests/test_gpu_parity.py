@@ -172,10 +172,11 @@ def test_ragged_batch_edge_cases(gp, ref, nbins):
 
 @pytest.mark.parametrize("nbins", [64, 256, 512, 1024])
 def test_packed_counts_long_and_short_curves(gp, ref, nbins):
-    """The fast kernels pack two 16-bit counts in one word (two rows at nbins 512 / 1024, two
-    period slots at nbins <= 256), which holds for curves of up to 65,535 samples; a longer
-    curve in the same batch is folded by a second launch (unpacked / generic kernel).  Cadence-locked
-    periods put thousands of samples in one bin."""
+    """fold_pk (nbins 512 ... 4096) packs the counts of rows k and k + rows/2 in the two
+    half-words of one word, which cannot wrap for curves of up to 65,535 samples; longer curves
+    in the same batch are folded without a flush first, checked, and folded again with the counts
+    flushed to a 32-bit side array only if a half-word wrapped (fold_lp, nbins <= 256, keeps
+    32-bit counts).  Cadence-locked periods put thousands of samples in one bin."""
     rng = np.random.default_rng(11)
     dt = workloads.KEPLER_CADENCE_D
     curves = []
