@@ -79,6 +79,14 @@ def test_host_side_validation_without_gpu(lib):
     assert lib.gpfc_fold_batch(None, None, None, 0, 0, None, 4, 64, None, None, None, None) == 0
     lib.gpfc_fold_batch_host.argtypes = fb
     assert lib.gpfc_fold_batch_host(None, None, None, 2, 10, None, 4, 64, None, None, None, None) == 1
+    # gpfc_fold_noalloc refuses sizes beyond its static scratch before it touches the device
+    lib.gpfc_fold_noalloc.argtypes = [vp, vp, i64, vp, i64, i32, f64, vp, vp, vp]
+    assert lib.gpfc_fold_noalloc(None, None, 131073, None, 8, 64, 0.0, None, None, None) == 2
+    assert b"GPFC_NOALLOC_MAX_SAMPLES" in lib.gpfc_last_error()
+    assert lib.gpfc_fold_noalloc(None, None, 100, None, 262145, 64, 0.0, None, None, None) == 2
+    assert b"GPFC_NOALLOC_MAX_PERIODS" in lib.gpfc_last_error()
+    assert lib.gpfc_fold_noalloc(None, None, -1, None, 8, 64, 0.0, None, None, None) == 1
+    assert lib.gpfc_fold_noalloc(None, None, 100, None, 8, 0, 0.0, None, None, None) == 2
     lib.gpfc_set_workspace.argtypes = [vp, ctypes.c_size_t]
     assert lib.gpfc_set_workspace(None, 16) == 1
     assert lib.gpfc_set_workspace(None, 0) == 0
