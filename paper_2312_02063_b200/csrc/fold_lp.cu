@@ -151,29 +151,38 @@ __device__ __forceinline__ unsigned pp_addr(double v, double rp, double C, unsig
     return addr;
 }
 
-// one sample at the lane's LP_R periods: the three sums first, then the three counts (measured:
-// the pair of atomics of one row back to back is ~1 % slower)
-template <bool IMM, bool GEN>
+// one sample at the lane's periods: the sums first, then the counts (measured: the pair of
+// atomics of one row back to back is ~1 % slower).  NR = period slots of the work item that hold
+// periods: LP_R for the items of fold_lp_kernel, 1 for those of fold_lp_tail_kernel.
+template <int NR, bool IMM, bool GEN>
 __device__ __forceinline__ void sample_update(double v, int q, const double (&rp)[LP_R],
                                               const double (&C)[LP_R], unsigned lane4,
                                               unsigned sbase, unsigned (&gmin)[LP_R], unsigned nbu)
 {
-    static_assert(LP_R == 3, "written out for three period slots");
+    static_assert(LP_R == 3 && (NR == 1 || NR == 3), "written out for one or three period slots");
     constexpr int B = IMM ? (int)LP_WINDOW_BASE : 0;
     const unsigned a0 = pp_addr<IMM, GEN>(v, rp[0], C[0], lane4, sbase, gmin[0], nbu);
-    const unsigned a1 = pp_addr<IMM, GEN>(v, rp[1], C[1], lane4, sbase, gmin[1], nbu);
-    const unsigned a2 = pp_addr<IMM, GEN>(v, rp[2], C[2], lane4, sbase, gmin[2], nbu);
-    red_add<B>(a0, q);
-    red_add<B + 65536>(a1, q);
-    red_add<B + 131072>(a2, q);
-    red_inc<B + 128>(a0);
-    red_inc<B + 65536 + 128>(a1);
-    red_inc<B + 131072 + 128>(a2);
+    if constexpr (NR == 3) {
+        const unsigned a1 = pp_addr<IMM, GEN>(v, rp[1], C[1], lane4, sbase, gmin[1], nbu);
+        const unsigned a2 = pp_addr<IMM, GEN>(v, rp[2], C[2], lane4, sbase, gmin[2], nbu);
+        red_add<B>(a0, q);
+        red_add<B + 65536>(a1, q);
+        red_add<B + 131072>(a2, q);
+        red_inc<B + 128>(a0);
+        red_inc<B + 65536 + 128>(a1);
+        red_inc<B + 131072 + 128>(a2);
+    } else {
+        red_add<B>(a0, q);
+        red_inc<B + 128>(a0);
+    }
 }
 
-template <bool IMM, bool GEN>
-__device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroups, long long nitems,
-                                             unsigned char *smem, unsigned sbase)
+// NR = LP_R: work items 0 .. nitems - 1 are (curve, group of LP_GROUP periods).
+// NR = 1 (fold_lp_tail_kernel): the groups from `first` on, cut into single period slots of 32
+// periods, nitems = LP_R x groups; only slot 0 of the histogram, 8 of the 24 warps in the epilogue.
+template <bool IMM, bool GEN, int NR>
+__device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroups, long long first,
+                                             long long nitems, unsigned char *smem, unsigned sbase)
 {
     unsigned *H = reinterpret_cast<unsigned *>(smem);
     double *ps1 = reinterpret_cast<double *>(smem + LP_PS1_OFF);
@@ -206,8 +215,19 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
     const bool vec = a.vec_ok != 0;
 
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
-        const long long curve = item / ngroups;
-        const long long p0 = (item - curve * ngroups) * LP_GROUP;
+        long long curve, p0, pend;                                   // pend: end of the item's periods
+        if constexpr (NR == LP_R) {
+            curve = item / ngroups;
+            p0 = (item - curve * ngroups) * LP_GROUP;
+            pend = a.nperiods;
+        } else {
+            const long long grp = first + item / LP_R;
+            curve = grp / ngroups;
+            p0 = (grp - curve * ngroups) * LP_GROUP + 32 * (item % LP_R);
+            pend = p0 + 32 * NR;
+            if (pend > a.nperiods) pend = a.nperiods;
+            if (pend <= p0) continue;                                // a slot past the last period
+        }
         const CurveMeta cm = a.meta[curve];
         const int n = cm.n_valid;
         const int ntiles = (n + GPFC_TILE - 1) / GPFC_TILE;
@@ -219,7 +239,7 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
 #pragma unroll
         for (int r = 0; r < LP_R; ++r) {
             long long j = p0 + r * 32 + lane;
-            double x = (j < a.nperiods) ? a.rp[j] : CUDART_NAN;
+            double x = (j < pend) ? a.rp[j] : CUDART_NAN;
             valid[r] = (x == x);
             rp[r] = valid[r] ? x : (double)LP_ROWS;   // dummy period: its columns are never written out
             if (valid[r]) rpmax = fmax(rpmax, x);
@@ -286,17 +306,17 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
 #pragma unroll(LP_UNROLL_C)
                         for (int s = 0; s < LP_GRAN / 2; s += 2) {
                             const int4 ra = stage[s], rb = stage[s + 1];
-                            sample_update<IMM, GEN>((double)(unsigned)ra.x, ra.y, rps, C, lane4, sbase, gmin, nbu);
-                            sample_update<IMM, GEN>((double)(unsigned)ra.z, ra.w, rps, C, lane4, sbase, gmin, nbu);
-                            sample_update<IMM, GEN>((double)(unsigned)rb.x, rb.y, rps, C, lane4, sbase, gmin, nbu);
-                            sample_update<IMM, GEN>((double)(unsigned)rb.z, rb.w, rps, C, lane4, sbase, gmin, nbu);
+                            sample_update<NR, IMM, GEN>((double)(unsigned)ra.x, ra.y, rps, C, lane4, sbase, gmin, nbu);
+                            sample_update<NR, IMM, GEN>((double)(unsigned)ra.z, ra.w, rps, C, lane4, sbase, gmin, nbu);
+                            sample_update<NR, IMM, GEN>((double)(unsigned)rb.x, rb.y, rps, C, lane4, sbase, gmin, nbu);
+                            sample_update<NR, IMM, GEN>((double)(unsigned)rb.z, rb.w, rps, C, lane4, sbase, gmin, nbu);
                         }
                     } else {
                         const int2 *st2 = reinterpret_cast<const int2 *>(stage);
 #pragma unroll 1
                         for (int s = 0; s < gc; ++s) {
                             const int2 rc = st2[s];
-                            sample_update<IMM, GEN>((double)(unsigned)rc.x, rc.y, rps, C, lane4, sbase, gmin, nbu);
+                            sample_update<NR, IMM, GEN>((double)(unsigned)rc.x, rc.y, rps, C, lane4, sbase, gmin, nbu);
                         }
                     }
                 }
@@ -369,7 +389,7 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
         }
         // the samples at u == 0 (CurveMeta::n_zero) are not in the sample arrays: bin 0 of every
         // period (atomics: other warps may still be folding)
-        if (warp < LP_R && cm.n_zero > 0) {
+        if (warp < NR && cm.n_zero > 0) {
             atomicAdd(&H[hidx(warp, 0, 0, lane)], (unsigned)cm.q_zero);
             atomicAdd(&H[hidx(warp, 0, 1, lane)], (unsigned)cm.n_zero);
         }
@@ -383,11 +403,13 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
         const double pivot_q = __dmul_rn(pivot, __ddiv_rn(1.0, inv_scale));   // in units of 2^-s: exact
         const double center_s = a.center_out ? 0.0 : center;       // FoldArgs::center_out: centred sums
         if (a.center_out && p0 == 0 && tid == 0) a.center_out[curve] = center;
-        const int octs = (nb + 7) >> 3;               // GEN: the last octet may be partial
+        // GEN: the last octet may be partial; a period slot the item does not use was never
+        // touched: nothing to write, nothing to clear
+        const int octs = (warp / LP_WPR < NR) ? ((nb + 7) >> 3) : 0;
         const bool vec8 = vec && !(nb & 7);
         const int r = warp / LP_WPR, wr = warp - r * LP_WPR;
         const long long j = p0 + r * 32 + lane;
-        const bool live = j < a.nperiods;
+        const bool live = j < pend;
         bool ok = false;
 #pragma unroll
         for (int rr = 0; rr < LP_R; ++rr)
@@ -504,7 +526,7 @@ __device__ __forceinline__ void fold_lp_body(const FoldArgs &a, long long ngroup
         }
         if (want_norm) {
             __syncthreads();
-            if (warp < LP_R) {
+            if (warp < NR) {
                 double s1 = 0.0, s2 = 0.0;
                 int kk = 0;
                 for (int w = 0; w < LP_WPR; ++w) {          // fixed order: deterministic
@@ -580,9 +602,22 @@ fold_lp_kernel(FoldArgs a, long long ngroups, long long nitems)
     extern __shared__ __align__(1024) unsigned char smem[];
     const unsigned sbase = (unsigned)__cvta_generic_to_shared(smem);
     if (sbase == LP_WINDOW_BASE)
-        fold_lp_body<true, GEN>(a, ngroups, nitems, smem, sbase);
+        fold_lp_body<true, GEN, LP_R>(a, ngroups, 0, nitems, smem, sbase);
     else
-        fold_lp_body<false, GEN>(a, ngroups, nitems, smem, sbase);
+        fold_lp_body<false, GEN, LP_R>(a, ngroups, 0, nitems, smem, sbase);
+}
+
+// the groups of a launch's last, partly filled wave, as single-slot items (launch_fold_lp)
+template <bool GEN>
+__global__ void __launch_bounds__(LP_THREADS, 1)
+fold_lp_tail_kernel(FoldArgs a, long long ngroups, long long first, long long nitems)
+{
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(smem);
+    if (sbase == LP_WINDOW_BASE)
+        fold_lp_body<true, GEN, 1>(a, ngroups, first, nitems, smem, sbase);
+    else
+        fold_lp_body<false, GEN, 1>(a, ngroups, first, nitems, smem, sbase);
 }
 
 }  // namespace
@@ -600,19 +635,44 @@ cudaError_t fold_lp_init_device()
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(fold_lp_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  LP_SMEM_BYTES);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(fold_lp_tail_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 LP_SMEM_BYTES);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(fold_lp_tail_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 LP_SMEM_BYTES);
     return e;
 }
 
 cudaError_t launch_fold_lp(const FoldArgs &a, cudaStream_t st, int sms)
 {
     const long long ngroups = (a.nperiods + LP_GROUP - 1) / LP_GROUP;
-    const long long nitems = ngroups * a.ncurves;
-    const long long grid = nitems < sms ? nitems : sms;
-    if (fold_lp_pow2(a.nbins))
-        fold_lp_kernel<false><<<(unsigned)grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems);
-    else
-        fold_lp_kernel<true><<<(unsigned)grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nitems);
-    note_launch();
+    const long long n3 = ngroups * a.ncurves;
+    // The CTAs take the items round robin, so the last wave of a launch holds n3 mod sms items
+    // while the other SMs idle for a whole item (config 1: 12 of 148 in wave 15 of 15).  When
+    // those groups, cut into single period slots, fit one wave, they go to fold_lp_tail_kernel
+    // instead (a single-slot item takes ~0.4 of a full one); so does a call of fewer groups
+    // than a third of the SMs.  The main kernel's code is the same with or without a tail.
+    const long long rem = n3 % sms;
+    const long long ntail = (rem > 0 && rem * LP_R <= sms) ? rem : 0;
+    const long long nreg = n3 - ntail;
+    const bool pow2 = fold_lp_pow2(a.nbins);
+    if (nreg > 0) {
+        const unsigned grid = (unsigned)(nreg < sms ? nreg : sms);
+        if (pow2)
+            fold_lp_kernel<false><<<grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nreg);
+        else
+            fold_lp_kernel<true><<<grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nreg);
+        note_launch();
+    }
+    if (ntail > 0) {
+        const unsigned grid = (unsigned)(ntail * LP_R);
+        if (pow2)
+            fold_lp_tail_kernel<false><<<grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nreg, ntail * LP_R);
+        else
+            fold_lp_tail_kernel<true><<<grid, LP_THREADS, LP_SMEM_BYTES, st>>>(a, ngroups, nreg, ntail * LP_R);
+        note_launch();
+    }
     return cudaGetLastError();
 }
 
