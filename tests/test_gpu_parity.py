@@ -577,7 +577,8 @@ def test_normalised_profile_does_not_depend_on_the_flux_scale(gp, ref, nbins):
 @pytest.mark.parametrize("nbins,nperiods", [(256, 14500), (100, 14500), (128, 96 * 148 + 1), (256, 96 * 148)])
 def test_item_counts_around_one_wave(gp, ref, nbins, nperiods):
     """One curve over a few more than 148 work items of 96 periods (a second, nearly empty
-    wave of the persistent grid), a last group of a single period, exactly 148 items."""
+    wave of the persistent grid: those groups run as single-slot items of fold_lp_tail_kernel),
+    a last group of a single period, exactly 148 items (no tail kernel)."""
     w = workloads.config1(nperiods=8)
     n = 3000
     periods = ref.make_period_grid(0.2, 1.0, nperiods)
