@@ -587,3 +587,47 @@ def test_item_counts_around_one_wave(gp, ref, nbins, nperiods):
     g = run_gpu(gp, ws, periods)
     r = ref.fold_batch(ws.times, ws.flux, ws.offsets, periods, nbins)
     check(g, r, exact_sums=True)
+
+
+@pytest.mark.parametrize("nbins", [64, 100, 256])
+def test_edge_cases_through_the_main_fold_lp_kernel(gp, ref, nbins):
+    """Calls of fewer than ~50 work items run entirely on fold_lp_tail_kernel (single-slot
+    items), which is where the small edge-case tests above end up.  The same edge cases with
+    enough periods for whole waves of three-slot items on fold_lp_kernel: the ragged batch
+    (empty and tiny curves, NaN samples, negative t - t0, per-curve t0, invalid and extreme
+    periods), flat and sparse profiles, 4-byte-aligned outputs."""
+    w = workloads.ragged_batch(nbins=nbins)
+    nper = 96 * (148 // w.ncurves + 2) + 5            # > 148 items, a partial last group per curve
+    periods = ref.make_period_grid(0.2, 3.0, nper, workloads.GRID_UNIFORM_PERIOD)
+    periods[[3, 200, nper - 1]] = np.nan
+    periods[[4, 97]] = [0.0, -0.5]
+    periods[[7, 300]] = [1e-9, 1e9]
+    periods[9] = 1e-320
+    t0 = np.linspace(-1.0, 2.0, w.ncurves)
+    ws = dataclasses.replace(w, nperiods=nper)
+    g = run_gpu(gp, ws, periods, t0=t0)
+    r = ref.fold_batch(w.times, w.flux, w.offsets, periods, nbins, t0=t0)
+    check(g, r)
+    c = gp.gpfc_path_counters()
+    assert c["generic_kernel_calls"] == 0
+    # flat / sparse profiles, outputs at offset 4 bytes
+    t = np.arange(3000, dtype=np.float64) * 0.0137
+    curves = [(t, np.full(3000, np.float32(3.0 * 2.0 ** -12)), None),
+              (np.array([0.3, 0.9]), np.array([1.0, -1.0], np.float32) * np.float32(2.0 ** -10), None),
+              (np.array([0.3]), np.array([2.0 ** -9], np.float32), None)]
+    nper2 = 96 * 52
+    p2 = ref.make_period_grid(0.25, 1.0, nper2)
+    wf = workloads._pack("flat", -1, curves, 0.25, 1.0, nper2, nbins, False)
+    r2 = ref.fold_batch(wf.times, wf.flux, wf.offsets, p2, nbins)
+    shape = (wf.ncurves, nper2, nbins)
+    nel = int(np.prod(shape))
+    bufs = [torch.zeros(nel + 3, dtype=dt, device="cuda") for dt in (torch.float32, torch.int32, torch.float32)]
+    os_, oc, on = (b[1:1 + nel].view(shape) for b in bufs)
+    gp.gpfc_fold_batch(dev(wf.times), dev(wf.flux), dev(wf.offsets), dev(p2), nbins,
+                       out_sum=os_, out_count=oc, out_norm=on)
+    torch.cuda.synchronize()
+    g2 = {"sum": os_.cpu().numpy(), "count": oc.cpu().numpy().view(np.uint32), "norm": on.cpu().numpy()}
+    check(g2, r2)
+    assert np.array_equal(g2["norm"][0], np.full_like(g2["norm"][0], np.float32(3.0 * 2.0 ** -12)))
+    for b in bufs:
+        assert float(b[0]) == 0 and float(b[nel + 1]) == 0
